@@ -1,0 +1,177 @@
+/*
+ * dnatok.h -- C-ABI of the B200-native DNATok hot path.
+ *
+ * Raw ASCII DNA bytes (FASTA-style records) -> token-ID streams on one GPU:
+ * 256-entry byte LUT (section 2.2 "bytes path"; Algorithm 1),
+ * newline / header stripping, then one of three vocabulary-agnostic encoders
+ * (single-nucleotide; non-overlapping k-mer, "length k, stride k", Alg. 1
+ * l.18 and PAPER.md:115-117 Alg. 2 l.7-8; BPE), CSR offsets,
+ * optional padding + attention mask (Alg. 2 l.12-14), and a pinned,
+ * multi-stream scheduler that overlaps the H2D copy of chunk i+1 with the encode of
+ * chunk i (section 2.2 "Pipelined streaming").  Everything the
+ * paper leaves open follows BASELINE.json north_star and the readings Q1-Q26 of
+ * SURVEY.md section 8(c), restated in DESIGN.md.
+ *
+ * Conventions
+ *   - plain C, no CUDA or torch types: a stream is passed as `void *` holding a
+ *     cudaStream_t (NULL = the legacy default stream); pointers named d_* are DEVICE
+ *     pointers, h_* are HOST pointers.
+ *   - every function returns a dnatok_status; nothing is thrown across the ABI.
+ *     dnatok_last_error() gives a human-readable message for the last failure on a
+ *     handle.
+ *   - the caller owns every input and output buffer.  The handle owns only what it
+ *     allocates itself (LUT copy, merge-rule hash, scan scratch, streaming slots);
+ *     dnatok_destroy() frees all of it.
+ *   - calls on ONE handle must be ordered with respect to each other (same stream, or
+ *     explicit event dependencies): the handle's scan scratch is not re-entrant.  Use
+ *     one handle per concurrent stream.
+ *   - there is no CPU fallback: every step runs in CUDA kernels for sm_100a.
+ *
+ * Class codes used by class_lut: 0..3 = A,C,G,T; 4 = N; 5 = UNK; 255 = SKIP (dropped).
+ */
+#ifndef DNATOK_H
+#define DNATOK_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct dnatok dnatok_t;   /* opaque */
+
+typedef enum {
+    DNATOK_OK = 0,
+    DNATOK_EINVAL = 1,      /* bad argument or configuration                                    */
+    DNATOK_ENOMEM = 2,      /* host or device allocation failed                                 */
+    DNATOK_ECUDA = 3,       /* a CUDA runtime call failed; see dnatok_last_error()              */
+    DNATOK_ECAPACITY = 4,   /* an output or carry buffer was too small; nothing written past it */
+    DNATOK_ESTATE = 5       /* internal scan protocol failure (look-back spin limit hit)        */
+} dnatok_status;
+
+enum { DNATOK_SINGLE_NT = 0, DNATOK_KMER = 1, DNATOK_BPE = 2 };               /* mode        */
+enum { DNATOK_I16 = 2, DNATOK_I32 = 4 };                                      /* id_dtype    */
+enum { DNATOK_TAIL_PER_BASE = 0, DNATOK_TAIL_DROP = 1, DNATOK_TAIL_UNK = 2 }; /* tail_policy */
+enum { DNATOK_PAD_LEFT = 0, DNATOK_PAD_RIGHT = 1 };                           /* pad_side    */
+
+#define DNATOK_CLS_N    4
+#define DNATOK_CLS_UNK  5
+#define DNATOK_CLS_SKIP 255
+#define DNATOK_MAX_K    15
+
+/*
+ * Create-time specification (vocabulary / LUT spec, k or merge table).
+ * Zero-initialise, set struct_size = sizeof(dnatok_config), then call
+ * dnatok_config_default() or fill the fields by hand.
+ */
+typedef struct {
+    uint32_t struct_size;     /* sizeof(dnatok_config); versioning                                         */
+    int32_t  mode;            /* DNATOK_SINGLE_NT | DNATOK_KMER | DNATOK_BPE                                */
+    int32_t  k;               /* KMER: window length 1..15 (ignored otherwise)                             */
+    int32_t  id_dtype;        /* DNATOK_I16 | DNATOK_I32: element type of ids_out.  I16 needs max id < 2^15 */
+    uint8_t  class_lut[256];  /* byte -> class code; all-zero => the default table (Aa Cc Gg Tt -> 0..3,    */
+                              /* Nn -> 4, '\n' '\r' -> SKIP, every other byte -> UNK)                       */
+    int32_t  strip_headers;   /* != 0: a line whose first byte is '>' is dropped through its '\n' (Q4).     */
+                              /* Requires class_lut['\n'] == SKIP.                                          */
+    int32_t  pad_id;          /* 0                                                                          */
+    int32_t  unk_id;          /* 1                                                                          */
+    int32_t  nt_ids[5];       /* SINGLE_NT: ids of A,C,G,T,N (2,3,4,5,6)                                    */
+    int32_t  base_id;         /* KMER: id = base_id + packed code; BPE: id = base_id + token (3)            */
+    int32_t  n_id;            /* BPE: id of an N byte (2)                                                   */
+    int32_t  tail_policy;     /* KMER: what the n mod k trailing bases become (Q9)                          */
+    const int32_t *merges;    /* BPE: HOST pointer to n_merges (left,right) pairs, copied at create;        */
+    int32_t  n_merges;        /*      rule r produces token 4 + r; parts must be < 4 + r, pairs unique (Q12) */
+    int32_t  seq_len;         /* pad: row length of batch_ids / mask; 0 => dnatok_pad unavailable           */
+    int32_t  pad_side;        /* DNATOK_PAD_LEFT (paper) | DNATOK_PAD_RIGHT                   */
+    int64_t  max_record_bytes;/* streaming / BPE: longest record in bytes the handle must be able to hold   */
+                              /* (carry buffer, per-read BPE workspace); 0 => 1 MiB                         */
+} dnatok_config;
+
+/* Fill *cfg with the BASELINE.json vocabulary (PAD 0, UNK 1, A..T 2..5, N 6; k-mer/BPE base_id 3, n_id 2),
+ * default LUT, strip_headers = 1, I32, PER_BASE tail, LEFT pad, seq_len 0.  mode and k as given.          */
+void dnatok_config_default(dnatok_config *cfg, int32_t mode, int32_t k);
+
+/*
+ * dnatok_create: validate cfg, select `device`, upload LUT / merge table, allocate scan scratch.
+ * EINVAL: k outside 1..15 (KMER); max id not fitting id_dtype; BPE rule referring to a token >= its own
+ * product or a duplicate pair; seq_len < 0; strip_headers with class_lut['\n'] != SKIP; class_lut entry
+ * not in {0..5, 255}.  On success *out owns the handle.
+ */
+int dnatok_create(const dnatok_config *cfg, int device, dnatok_t **out);
+int dnatok_destroy(dnatok_t *h);
+
+/*
+ * dnatok_encode: steps 1-5 (classify, strip, encode, CSR offsets) for n_records records.
+ *   d_bytes        [n_bytes] uint8, any alignment.  Record r is the byte range
+ *                  [d_rec_offsets[r], d_rec_offsets[r+1]).
+ *   d_rec_offsets  [n_records+1] int64, non-decreasing, 0 <= offsets[0], offsets[n_records] <= n_bytes
+ *                  (precondition, not checked).  Bytes outside every record are ignored.
+ *   d_ids_out      [ids_capacity] elements of id_dtype.  ids_capacity >= n_bytes always suffices
+ *                  (tokens <= kept bases <= bytes).  On overflow nothing is written past the end, the
+ *                  handle's status word is set and dnatok_check() returns DNATOK_ECAPACITY.
+ *   d_out_offsets  [n_records+1] int64: exclusive prefix sum of per-record token counts, total last.
+ * Only enqueues work on `stream`; never synchronises.
+ */
+int dnatok_encode(dnatok_t *h, const uint8_t *d_bytes, int64_t n_bytes,
+                  const int64_t *d_rec_offsets, int64_t n_records,
+                  void *d_ids_out, int64_t ids_capacity, int64_t *d_out_offsets, void *stream);
+
+/*
+ * dnatok_pad: step 6.  Row r of d_batch_ids [n_records][seq_len] (int32) gets record r's first
+ * min(tokens, seq_len) ids, LEFT: right-aligned, RIGHT: left-aligned; other columns pad_id.
+ * d_mask [n_records][seq_len] (uint8) is 1 exactly on the kept columns; may be NULL.
+ * d_ids / d_out_offsets are dnatok_encode's outputs (element type id_dtype).  Enqueue only.
+ */
+int dnatok_pad(dnatok_t *h, const void *d_ids, const int64_t *d_out_offsets, int64_t n_records,
+               int32_t *d_batch_ids, uint8_t *d_mask, void *stream);
+
+/* One delivered batch of dnatok_stream_encode (device pointers valid until the callback's stream work ends). */
+typedef struct {
+    int64_t first_record;        /* index of the first record in this batch                     */
+    int64_t n_records;           /* records that END in this chunk (Q17), in order              */
+    const void    *d_ids;        /* CSR ids (id_dtype) of these records                         */
+    const int64_t *d_out_offsets;/* [n_records+1], relative to this batch                       */
+    const int32_t *d_batch_ids;  /* [n_records][seq_len] or NULL when seq_len == 0              */
+    const uint8_t *d_mask;       /* [n_records][seq_len] or NULL when seq_len == 0              */
+    int64_t chunk_index;
+    void   *stream;              /* cudaStream_t the batch was produced on                      */
+} dnatok_batch;
+
+typedef void (*dnatok_batch_fn)(void *user, const dnatok_batch *batch);
+
+/*
+ * dnatok_stream_encode: step 7.  Splits the PINNED host buffer into chunk_bytes pieces; chunk i goes to
+ * device slot i mod n_streams on its own stream: H2D copy, carry of the record cut by the previous chunk
+ * boundary, steps 1-6.  H2D of chunk i+1 overlaps the encode of chunk i.  Output equals dnatok_encode
+ * (+ dnatok_pad) on the whole buffer, delivered batch by batch in record order; a record is delivered in
+ * the chunk where it ends.  on_batch is called on the calling thread right after the batch's work has been
+ * enqueued on batch->stream (enqueue consumer work there; the slot is recycled n_streams chunks later,
+ * after that stream's work).  Returns after the last chunk has completed.
+ *   h_pinned       [n_bytes] page-locked host memory (cudaHostAlloc / cudaHostRegister / torch pin_memory)
+ *   h_rec_offsets  [n_records+1] host int64, same contract as dnatok_encode
+ *   max_rows_per_chunk  upper bound on records ending in one chunk (sizes the per-slot batch tensors);
+ *                  0 => chunk_bytes / 64 + 2.  Exceeding it returns DNATOK_ECAPACITY.
+ * A record longer than cfg.max_record_bytes + chunk_bytes returns DNATOK_ECAPACITY.
+ */
+int dnatok_stream_encode(dnatok_t *h, const uint8_t *h_pinned, int64_t n_bytes,
+                         const int64_t *h_rec_offsets, int64_t n_records,
+                         int64_t chunk_bytes, int n_streams, int64_t max_rows_per_chunk,
+                         dnatok_batch_fn on_batch, void *user);
+
+/* Synchronise `stream` and report the handle's device status word: DNATOK_OK, DNATOK_ECAPACITY or
+ * DNATOK_ESTATE (sticky until read).                                                                  */
+int dnatok_check(dnatok_t *h, void *stream);
+
+/* Message for the last non-OK return on this handle (never NULL; valid until the next call on h).      */
+const char *dnatok_last_error(const dnatok_t *h);
+
+/* Number of kernels this library has launched on the handle since create (bench.py's gpu_launches).    */
+int64_t dnatok_launch_count(const dnatok_t *h);
+
+/* Library version string, e.g. "dnatok-b200 0.1 (sm_100a)".                                            */
+const char *dnatok_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* DNATOK_H */

@@ -1,0 +1,239 @@
+// bpe_kernel.cuh -- BPE merge kernel: one read per thread block, lowest rank first.
+//
+// Semantics: the kept classes of a read are cut at every
+// N / UNK (each is its own token and a hard boundary); inside each ACGT segment, repeat
+// { take the lowest-rank adjacent pair that has a rule; replace all its occurrences left to
+// right without overlap } until no adjacent pair has a rule.
+//
+// Parallel form: all segments of the read advance together, one "round" per iteration; in a
+// round every segment applies ITS OWN current minimum rank (segments never interact, so this
+// equals the sequential order segment by segment).  Merging every locally-minimal pair at once
+// would be wrong (SURVEY.md section 7 hard part 5), so only pairs whose rank equals the
+// segment minimum fire.  Pair ranks are cached next to the symbols and only pairs touching a
+// freshly merged token are looked up again (one hash probe sequence each).
+#pragma once
+#include "common.cuh"
+
+namespace dtk {
+
+constexpr int BPE_NT = 128;
+constexpr uint32_t BPE_INF = 0xffffu;          // "no rule" rank / also the largest uint16
+constexpr uint32_t SYM_N = 0xffffu, SYM_UNK = 0xfffeu;   // boundary symbols (never merged, never removed)
+constexpr uint64_t HASH_EMPTY = ~0ull;
+
+struct BpeArgs {
+    const uint8_t *cls;            // compact kept classes of all reads (pass A output)
+    const int64_t *koff;           // [n_rec + 1] kept-base CSR offsets (pass A output)
+    int64_t n_rec;
+    const uint64_t *table;         // open-addressing hash: (left<<16|right)<<32 | rank
+    uint32_t table_mask;
+    int32_t cap;                   // symbols per read the shared-memory workspace can hold
+    uint16_t *tmp_tok;             // token numbers of read r at tmp_tok[koff[r] ...)
+    int32_t *tok_cnt;              // [n_rec] tokens per read
+    uint32_t *status;
+};
+
+__device__ __forceinline__ uint32_t bpe_hash(uint32_t key) {
+    key ^= key >> 15; key *= 0x2c1b3c6du; key ^= key >> 12; key *= 0x297a2d39u; key ^= key >> 15;
+    return key;
+}
+
+__device__ __forceinline__ uint32_t bpe_rank(const BpeArgs &A, uint32_t l, uint32_t r) {
+    if (l >= SYM_UNK || r >= SYM_UNK) return BPE_INF;
+    const uint32_t key = (l << 16) | r;
+    uint32_t h = bpe_hash(key) & A.table_mask;
+    for (;;) {
+        uint64_t s = __ldg(A.table + h);
+        if (s == HASH_EMPTY) return BPE_INF;
+        if ((uint32_t)(s >> 32) == key) return (uint32_t)s;
+        h = (h + 1) & A.table_mask;
+    }
+}
+
+// block-wide exclusive scan (BPE_NT threads)
+__device__ __forceinline__ int bpe_exscan(int v, int *warp_tmp, int &total) {
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    int inc = v;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) { int t = __shfl_up_sync(0xffffffffu, inc, d); if (lane >= d) inc += t; }
+    if (lane == 31) warp_tmp[warp] = inc;
+    __syncthreads();
+    int woff = 0, tot = 0;
+#pragma unroll
+    for (int w = 0; w < BPE_NT / 32; ++w) { int t = warp_tmp[w]; if (w < warp) woff += t; tot += t; }
+    __syncthreads();
+    total = tot;
+    return woff + inc - v;
+}
+
+// dynamic shared memory layout: sym[2][cap] rnk[2][cap] seg[2][cap] src[cap] segmin[cap+1], all uint16
+__global__ void __launch_bounds__(BPE_NT) bpe_reads_kernel(const __grid_constant__ BpeArgs A) {
+    extern __shared__ __align__(16) uint16_t sh[];
+    __shared__ int warp_tmp[BPE_NT / 32];
+    __shared__ int s_any;
+    const int cap = A.cap, tid = threadIdx.x;
+    uint16_t *symb[2] = {sh, sh + cap};
+    uint16_t *rnkb[2] = {sh + 2 * cap, sh + 3 * cap};
+    uint16_t *segb[2] = {sh + 4 * cap, sh + 5 * cap};
+    uint16_t *src = sh + 6 * cap;
+    uint16_t *segmin = sh + 7 * cap;
+
+    for (int64_t r = blockIdx.x; r < A.n_rec; r += gridDim.x) {
+        const int64_t k0 = A.koff[r];
+        const int64_t n64 = A.koff[r + 1] - k0;
+        __syncthreads();
+        if (n64 > cap) {                      // read does not fit the workspace: report, emit nothing
+            if (tid == 0) { A.status[0] = 1u; A.tok_cnt[r] = 0; }
+            continue;
+        }
+        int n = (int)n64, cur = 0;
+        // ---- load symbols, segment ids (a boundary symbol forms its own segment) --------
+        // seg id = number of "segment starts" at or before i, minus 1; a start is i == 0, a boundary,
+        // or the position right after a boundary.
+        for (int base = 0; base < n; base += BPE_NT) {       // chunked so the scan carries across chunks
+            int i = base + tid;
+            uint32_t c = (i < n) ? A.cls[k0 + i] : 0u;
+            uint32_t s = c < CLS_N ? c : (c == CLS_N ? SYM_N : SYM_UNK);
+            if (i < n) symb[0][i] = (uint16_t)s;
+        }
+        __syncthreads();
+        int seg_base = 0;
+        for (int base = 0; base < n; base += BPE_NT) {
+            int i = base + tid;
+            int start = 0;
+            if (i < n) {
+                bool b = symb[0][i] >= SYM_UNK;
+                bool pb = (i > 0) && symb[0][i - 1] >= SYM_UNK;
+                start = (i == 0 || b || pb) ? 1 : 0;
+            }
+            int tot;
+            int ex = bpe_exscan(start, warp_tmp, tot);
+            if (i < n) segb[0][i] = (uint16_t)(seg_base + ex + start - 1);
+            seg_base += tot;
+        }
+        for (int i = tid; i < n; i += BPE_NT)
+            rnkb[0][i] = (uint16_t)((i + 1 < n) ? bpe_rank(A, symb[0][i], symb[0][i + 1]) : BPE_INF);
+        __syncthreads();
+
+        // ---- rounds ----------------------------------------------------------------------
+        for (;;) {
+            uint16_t *sym = symb[cur], *rnk = rnkb[cur], *seg = segb[cur];
+            uint16_t *sym2 = symb[cur ^ 1], *rnk2 = rnkb[cur ^ 1], *seg2 = segb[cur ^ 1];
+            if (tid == 0) s_any = 0;
+            for (int i = tid; i <= seg_base; i += BPE_NT) segmin[i] = (uint16_t)BPE_INF;
+            __syncthreads();
+            // per-segment minimum rank (16-bit values packed two per word: CAS-free atomicMin on the half)
+            bool any = false;
+            for (int i = tid; i < n; i += BPE_NT) {
+                uint32_t rk = rnk[i];
+                if (rk != BPE_INF) {
+                    any = true;
+                    uint32_t sg = seg[i];
+                    uint32_t *w = reinterpret_cast<uint32_t *>(segmin) + (sg >> 1);
+                    // min on one 16-bit half: try until our value is not smaller any more
+                    uint32_t old = *w;
+                    for (;;) {
+                        uint32_t half = (sg & 1) ? (old >> 16) : (old & 0xffffu);
+                        if (half <= rk) break;
+                        uint32_t neu = (sg & 1) ? ((old & 0xffffu) | (rk << 16)) : ((old & 0xffff0000u) | rk);
+                        uint32_t got = atomicCAS(w, old, neu);
+                        if (got == old) break;
+                        old = got;
+                    }
+                }
+            }
+            if (any) s_any = 1;
+            __syncthreads();
+            if (!s_any) break;
+            // flags, run parity, compaction
+            int carry = 0;
+            for (int base = 0; base < n; base += BPE_NT) {
+                int i = base + tid;
+                bool keep = false, merge = false;
+                if (i < n) {
+                    auto fires = [&](int j) -> bool {            // pair (j, j+1) is selected (before overlap rule)
+                        uint32_t rk = rnk[j];
+                        return rk != BPE_INF && rk == segmin[seg[j]];
+                    };
+                    auto merges = [&](int j) -> bool {           // left to right, non-overlapping (Q11)
+                        if (!fires(j)) return false;
+                        int c = 0;
+                        while (j - 1 - c >= 0 && fires(j - 1 - c)) ++c;
+                        return (c & 1) == 0;
+                    };
+                    merge = merges(i);
+                    keep = !(i > 0 && merges(i - 1));
+                }
+                int tot;
+                int w = carry + bpe_exscan(keep ? 1 : 0, warp_tmp, tot);
+                if (keep) {
+                    sym2[w] = merge ? (uint16_t)(4u + rnk[i]) : sym[i];
+                    seg2[w] = seg[i];
+                    src[w] = (uint16_t)(merge ? 0xffffu : i);    // 0xffff: freshly merged token
+                }
+                carry += tot;
+            }
+            __syncthreads();
+            const int n2 = carry;
+            for (int w = tid; w < n2; w += BPE_NT) {
+                uint32_t rk = BPE_INF;
+                if (w + 1 < n2) {
+                    if (src[w] == 0xffffu || src[w + 1] == 0xffffu) rk = bpe_rank(A, sym2[w], sym2[w + 1]);
+                    else rk = rnk[src[w]];
+                }
+                rnk2[w] = (uint16_t)rk;
+            }
+            n = n2; cur ^= 1;
+            __syncthreads();
+        }
+        // ---- write token numbers --------------------------------------------------------
+        for (int i = tid; i < n; i += BPE_NT) A.tmp_tok[k0 + i] = symb[cur][i];
+        if (tid == 0) A.tok_cnt[r] = n;
+    }
+}
+
+// single-block exclusive scan of per-read token counts -> out_offsets (int64), total in the last entry
+__global__ void __launch_bounds__(1024) scan_counts_kernel(const int32_t *cnt, int64_t n, int64_t *out_off) {
+    __shared__ long long wsum[32];
+    __shared__ long long s_carry;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    if (tid == 0) s_carry = 0;
+    __syncthreads();
+    for (int64_t base = 0; base < n; base += 1024) {
+        int64_t i = base + tid;
+        long long v = (i < n) ? cnt[i] : 0, inc = v;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) { long long t = __shfl_up_sync(0xffffffffu, inc, d); if (lane >= d) inc += t; }
+        if (lane == 31) wsum[warp] = inc;
+        __syncthreads();
+        long long woff = 0, tot = 0;
+        for (int w = 0; w < 32; ++w) { long long t = wsum[w]; if (w < warp) woff += t; tot += t; }
+        long long carry = s_carry;
+        if (i < n) out_off[i] = carry + woff + inc - v;
+        __syncthreads();
+        if (tid == 0) s_carry = carry + tot;
+        __syncthreads();
+    }
+    if (tid == 0) out_off[n] = s_carry;
+}
+
+template <typename IdT>
+__global__ void __launch_bounds__(256) bpe_gather_kernel(const uint16_t *tmp_tok, const int64_t *koff,
+                                                         const int64_t *out_off, int64_t n_rec, IdT *ids,
+                                                         int64_t ids_cap, int32_t base_id, int32_t n_id,
+                                                         int32_t unk_id, uint32_t *status) {
+    const int lane = threadIdx.x & 31;
+    const int64_t warp = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const int64_t nwarps = ((int64_t)gridDim.x * blockDim.x) >> 5;
+    for (int64_t r = warp; r < n_rec; r += nwarps) {
+        const int64_t k0 = koff[r], o0 = out_off[r];
+        const int n = (int)(out_off[r + 1] - o0);
+        for (int i = lane; i < n; i += 32) {
+            uint32_t s = tmp_tok[k0 + i];
+            int32_t id = s == SYM_N ? n_id : (s == SYM_UNK ? unk_id : (int32_t)(base_id + s));
+            if (o0 + i < ids_cap) ids[o0 + i] = (IdT)id; else status[0] = 1u;
+        }
+    }
+}
+
+}  // namespace dtk

@@ -1,0 +1,547 @@
+// dnatok_api.cu -- host side of the C-ABI declared in include/dnatok.h.
+//
+// Argument marshalling, scratch management and the pinned multi-stream scheduler; every
+// step of the hot path itself runs in the kernels of encode_kernel.cuh / bpe_kernel.cuh /
+// pad_kernel.cuh.  There is no CPU fallback anywhere in this file.
+#include "../../include/dnatok.h"
+
+#include <algorithm>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include "bpe_kernel.cuh"
+#include "common.cuh"
+#include "encode_kernel.cuh"
+#include "pad_kernel.cuh"
+
+using namespace dtk;
+
+namespace {
+
+// scan scratch of one in-flight encode: tile descriptors, ticket counter, host-mapped status words
+struct EncCtx {
+    TileDesc *descs = nullptr;
+    int64_t descs_cap = 0;
+    unsigned long long *ticket = nullptr;
+    unsigned long long ticket_base = 0;
+    uint32_t *h_status = nullptr;      // pinned + mapped: [0] capacity overflow, [1] scan protocol failure
+    uint32_t *d_status = nullptr;      // device alias of h_status
+    uint32_t gen = 0;
+    // BPE pass scratch
+    uint8_t *cls = nullptr;  int64_t cls_cap = 0;
+    uint16_t *tmp_tok = nullptr;
+    int64_t *koff = nullptr; int32_t *tok_cnt = nullptr; int64_t rec_cap = 0;
+};
+
+struct StreamSlot {
+    uint8_t *d_buf = nullptr;
+    int64_t *d_recoff = nullptr, *h_recoff = nullptr;
+    void *d_ids = nullptr;
+    int64_t *d_out_off = nullptr;
+    int32_t *d_batch = nullptr;
+    uint8_t *d_mask = nullptr;
+    cudaEvent_t ev_h2d = nullptr, ev_carry = nullptr, ev_done = nullptr, ev_off = nullptr;
+    EncCtx ctx;
+};
+
+struct StreamRing {
+    int64_t chunk_bytes = 0, carry_cap = 0, max_rows = 0;
+    int n_streams = 0, n_slots = 0;
+    std::vector<cudaStream_t> streams;
+    std::vector<StreamSlot> slots;
+};
+
+}  // namespace
+
+struct dnatok {
+    dnatok_config cfg;
+    int device = 0;
+    int sm_count = 0;
+    EncParams prm;
+    uint8_t *d_lut = nullptr;
+    uint64_t *d_table = nullptr;
+    uint32_t table_mask = 0;
+    int32_t bpe_cap = 0;
+    EncCtx ctx;
+    StreamRing ring;
+    int enc_ctas_per_sm = 1, bpe_ctas_per_sm = 1;
+    int64_t launches = 0;
+    std::string err;
+};
+
+namespace {
+
+int fail(dnatok_t *h, int code, const char *fmt, ...) {
+    if (h) {
+        char buf[512];
+        va_list ap; va_start(ap, fmt); vsnprintf(buf, sizeof buf, fmt, ap); va_end(ap);
+        h->err = buf;
+    }
+    return code;
+}
+
+#define CU(call)                                                                                      \
+    do {                                                                                              \
+        cudaError_t e_ = (call);                                                                      \
+        if (e_ != cudaSuccess)                                                                        \
+            return fail(h, e_ == cudaErrorMemoryAllocation ? DNATOK_ENOMEM : DNATOK_ECUDA, "%s: %s", \
+                        #call, cudaGetErrorString(e_));                                               \
+    } while (0)
+
+void default_lut(uint8_t *lut) {
+    for (int b = 0; b < 256; ++b) lut[b] = DNATOK_CLS_UNK;
+    const char *up = "ACGTN", *lo = "acgtn";
+    for (int i = 0; i < 5; ++i) { lut[(uint8_t)up[i]] = (uint8_t)i; lut[(uint8_t)lo[i]] = (uint8_t)i; }
+    lut['\n'] = DNATOK_CLS_SKIP; lut['\r'] = DNATOK_CLS_SKIP;
+}
+
+uint32_t host_hash(uint32_t key) {   // must match bpe_hash()
+    key ^= key >> 15; key *= 0x2c1b3c6du; key ^= key >> 12; key *= 0x297a2d39u; key ^= key >> 15;
+    return key;
+}
+
+int ctx_init(dnatok_t *h, EncCtx &c) {
+    CU(cudaMalloc(&c.ticket, sizeof(unsigned long long)));
+    CU(cudaMemset(c.ticket, 0, sizeof(unsigned long long)));
+    CU(cudaHostAlloc(&c.h_status, 2 * sizeof(uint32_t), cudaHostAllocMapped));
+    c.h_status[0] = c.h_status[1] = 0;
+    CU(cudaHostGetDevicePointer((void **)&c.d_status, c.h_status, 0));
+    return DNATOK_OK;
+}
+
+void ctx_free(EncCtx &c) {
+    cudaFree(c.descs); cudaFree(c.ticket); cudaFreeHost(c.h_status);
+    cudaFree(c.cls); cudaFree(c.tmp_tok); cudaFree(c.koff); cudaFree(c.tok_cnt);
+    c = EncCtx();
+}
+
+// stream-ordered growth of the tile-descriptor array (never synchronises the host)
+int ctx_reserve_tiles(dnatok_t *h, EncCtx &c, int64_t n_tiles, cudaStream_t st) {
+    if (n_tiles <= c.descs_cap) return DNATOK_OK;
+    int64_t cap = std::max<int64_t>(n_tiles + n_tiles / 4, 1024);
+    if (c.descs) CU(cudaFreeAsync(c.descs, st));
+    c.descs = nullptr; c.descs_cap = 0;
+    CU(cudaMallocAsync((void **)&c.descs, (size_t)cap * sizeof(TileDesc), st));
+    CU(cudaMemsetAsync(c.descs, 0, (size_t)cap * sizeof(TileDesc), st));
+    c.descs_cap = cap;
+    return DNATOK_OK;
+}
+
+int ctx_next_gen(dnatok_t *h, EncCtx &c, cudaStream_t st) {
+    if (++c.gen >= (1u << 24) - 1) {       // generation tags are 24 bits wide in TileDesc::l_word
+        if (c.descs) CU(cudaMemsetAsync(c.descs, 0, (size_t)c.descs_cap * sizeof(TileDesc), st));
+        c.gen = 1;
+    }
+    return DNATOK_OK;
+}
+
+template <typename IdT>
+int launch_tiles(dnatok_t *h, EncCtx &c, const EncParams &prm, const uint8_t *d_bytes, int64_t n_bytes,
+                 const int64_t *d_rec_off, int64_t n_rec, int64_t off_bias, void *ids, int64_t ids_cap,
+                 int64_t *out_off, cudaStream_t st) {
+    EncArgs a;
+    uintptr_t addr = reinterpret_cast<uintptr_t>(d_bytes);
+    a.mis = (int64_t)(addr & 15);
+    a.bytes_al = reinterpret_cast<const uint8_t *>(addr - (uintptr_t)a.mis);
+    a.p_end = a.mis + n_bytes;
+    int64_t n_tiles = a.p_end / TB + 1;
+    if (n_tiles > 0x7fffffff) return fail(h, DNATOK_EINVAL, "n_bytes too large for one call");
+    int rc = ctx_reserve_tiles(h, c, n_tiles, st); if (rc) return rc;
+    rc = ctx_next_gen(h, c, st); if (rc) return rc;
+    a.rec_off = d_rec_off; a.n_rec = n_rec; a.off_bias = off_bias;
+    a.ids = ids; a.ids_cap = ids_cap; a.out_off = out_off; a.out_bias = 0;
+    a.lut = h->d_lut; a.descs = c.descs; a.ticket = c.ticket; a.ticket_base = c.ticket_base;
+    a.status = c.d_status; a.gen = c.gen; a.n_tiles = (int32_t)n_tiles; a.prm = prm;
+    int grid = (int)std::min<int64_t>(n_tiles, (int64_t)h->sm_count * h->enc_ctas_per_sm);
+    encode_tiles_kernel<IdT><<<grid, NT, sizeof(TileSmem), st>>>(a);
+    CU(cudaGetLastError());
+    c.ticket_base += (unsigned long long)n_tiles + (unsigned long long)grid;
+    h->launches += 1;
+    return DNATOK_OK;
+}
+
+int ctx_reserve_bpe(dnatok_t *h, EncCtx &c, int64_t n_bytes, int64_t n_rec, cudaStream_t st) {
+    if (n_bytes > c.cls_cap) {
+        int64_t cap = n_bytes + n_bytes / 8 + 256;
+        if (c.cls) CU(cudaFreeAsync(c.cls, st));
+        if (c.tmp_tok) CU(cudaFreeAsync(c.tmp_tok, st));
+        c.cls = nullptr; c.tmp_tok = nullptr; c.cls_cap = 0;
+        CU(cudaMallocAsync((void **)&c.cls, (size_t)cap, st));
+        CU(cudaMallocAsync((void **)&c.tmp_tok, (size_t)cap * sizeof(uint16_t), st));
+        c.cls_cap = cap;
+    }
+    if (n_rec + 1 > c.rec_cap) {
+        int64_t cap = n_rec + n_rec / 8 + 256;
+        if (c.koff) CU(cudaFreeAsync(c.koff, st));
+        if (c.tok_cnt) CU(cudaFreeAsync(c.tok_cnt, st));
+        c.koff = nullptr; c.tok_cnt = nullptr; c.rec_cap = 0;
+        CU(cudaMallocAsync((void **)&c.koff, (size_t)cap * sizeof(int64_t), st));
+        CU(cudaMallocAsync((void **)&c.tok_cnt, (size_t)cap * sizeof(int32_t), st));
+        c.rec_cap = cap;
+    }
+    return DNATOK_OK;
+}
+
+size_t bpe_smem_bytes(int cap) { return (size_t)(8 * cap + 8) * sizeof(uint16_t); }
+
+int encode_on(dnatok_t *h, EncCtx &c, const uint8_t *d_bytes, int64_t n_bytes, const int64_t *d_rec_off,
+              int64_t n_rec, int64_t off_bias, void *d_ids, int64_t ids_cap, int64_t *d_out_off, cudaStream_t st) {
+    const dnatok_config &cfg = h->cfg;
+    if (cfg.mode != DNATOK_BPE) {
+        if (cfg.id_dtype == DNATOK_I16)
+            return launch_tiles<int16_t>(h, c, h->prm, d_bytes, n_bytes, d_rec_off, n_rec, off_bias, d_ids, ids_cap, d_out_off, st);
+        return launch_tiles<int32_t>(h, c, h->prm, d_bytes, n_bytes, d_rec_off, n_rec, off_bias, d_ids, ids_cap, d_out_off, st);
+    }
+    // BPE: pass A = compact kept classes + kept-base CSR offsets (the single-nt encoder with class ids),
+    //      pass B = merge kernel per read, pass C = offsets scan, pass D = gather into ids_out
+    int rc = ctx_reserve_bpe(h, c, n_bytes, n_rec, st); if (rc) return rc;
+    EncParams pa = h->prm;
+    pa.mode = MODE_SINGLE_NT; pa.k = 1; pa.unk_id = DNATOK_CLS_UNK;
+    for (int i = 0; i < 5; ++i) pa.nt_ids[i] = i;
+    rc = launch_tiles<uint8_t>(h, c, pa, d_bytes, n_bytes, d_rec_off, n_rec, off_bias, c.cls, c.cls_cap, c.koff, st);
+    if (rc) return rc;
+    if (n_rec > 0) {
+        BpeArgs b;
+        b.cls = c.cls; b.koff = c.koff; b.n_rec = n_rec; b.table = h->d_table; b.table_mask = h->table_mask;
+        b.cap = h->bpe_cap; b.tmp_tok = c.tmp_tok; b.tok_cnt = c.tok_cnt; b.status = c.d_status;
+        int grid = (int)std::min<int64_t>(n_rec, (int64_t)h->sm_count * h->bpe_ctas_per_sm);
+        bpe_reads_kernel<<<grid, BPE_NT, bpe_smem_bytes(h->bpe_cap), st>>>(b);
+        CU(cudaGetLastError());
+        h->launches += 1;
+    }
+    scan_counts_kernel<<<1, 1024, 0, st>>>(c.tok_cnt, n_rec, d_out_off);
+    CU(cudaGetLastError());
+    h->launches += 1;
+    if (n_rec > 0) {
+        int grid = (int)std::min<int64_t>((n_rec + 7) / 8, (int64_t)h->sm_count * 8);
+        if (cfg.id_dtype == DNATOK_I16)
+            bpe_gather_kernel<int16_t><<<grid, 256, 0, st>>>(c.tmp_tok, c.koff, d_out_off, n_rec, (int16_t *)d_ids, ids_cap,
+                                                           cfg.base_id, cfg.n_id, cfg.unk_id, c.d_status);
+        else
+            bpe_gather_kernel<int32_t><<<grid, 256, 0, st>>>(c.tmp_tok, c.koff, d_out_off, n_rec, (int32_t *)d_ids, ids_cap,
+                                                           cfg.base_id, cfg.n_id, cfg.unk_id, c.d_status);
+        CU(cudaGetLastError());
+        h->launches += 1;
+    }
+    return DNATOK_OK;
+}
+
+int pad_on(dnatok_t *h, const void *d_ids, const int64_t *d_out_off, int64_t n_rec, int32_t *d_batch,
+           uint8_t *d_mask, cudaStream_t st) {
+    if (n_rec == 0) return DNATOK_OK;
+    PadArgs a;
+    a.ids = d_ids; a.out_off = d_out_off; a.n_rows = n_rec; a.batch_ids = d_batch; a.mask = d_mask;
+    a.seq_len = h->cfg.seq_len; a.pad_side = h->cfg.pad_side; a.pad_id = h->cfg.pad_id;
+    int grid = (int)std::min<int64_t>(n_rec, (int64_t)h->sm_count * 16);
+    if (h->cfg.id_dtype == DNATOK_I16) pad_rows_kernel<int16_t><<<grid, 256, 0, st>>>(a);
+    else pad_rows_kernel<int32_t><<<grid, 256, 0, st>>>(a);
+    CU(cudaGetLastError());
+    h->launches += 1;
+    return DNATOK_OK;
+}
+
+int status_of(dnatok_t *h, EncCtx &c) {
+    int rc = DNATOK_OK;
+    if (c.h_status[1]) rc = fail(h, DNATOK_ESTATE, "scan look-back spin limit hit (tile chain broken)");
+    else if (c.h_status[0]) rc = fail(h, DNATOK_ECAPACITY, "an output buffer or workspace was too small");
+    c.h_status[0] = c.h_status[1] = 0;
+    return rc;
+}
+
+void ring_free(StreamRing &r) {
+    for (auto &s : r.slots) {
+        cudaFree(s.d_buf); cudaFree(s.d_recoff); cudaFreeHost(s.h_recoff); cudaFree(s.d_ids); cudaFree(s.d_out_off);
+        cudaFree(s.d_batch); cudaFree(s.d_mask);
+        if (s.ev_h2d) cudaEventDestroy(s.ev_h2d);
+        if (s.ev_carry) cudaEventDestroy(s.ev_carry);
+        if (s.ev_done) cudaEventDestroy(s.ev_done);
+        if (s.ev_off) cudaEventDestroy(s.ev_off);
+        ctx_free(s.ctx);
+    }
+    for (auto st : r.streams) cudaStreamDestroy(st);
+    r = StreamRing();
+}
+
+int ring_setup(dnatok_t *h, int64_t chunk_bytes, int n_streams, int64_t max_rows) {
+    StreamRing &r = h->ring;
+    const int64_t carry_cap = (h->cfg.max_record_bytes + 255) & ~(int64_t)255;
+    if (r.chunk_bytes == chunk_bytes && r.n_streams == n_streams && r.max_rows >= max_rows && r.carry_cap == carry_cap)
+        return DNATOK_OK;
+    ring_free(r);
+    r.chunk_bytes = chunk_bytes; r.n_streams = n_streams; r.n_slots = std::max(2, n_streams);
+    r.max_rows = max_rows; r.carry_cap = carry_cap;
+    r.streams.resize(n_streams);
+    for (auto &st : r.streams) CU(cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking));
+    r.slots.resize(r.n_slots);
+    const int64_t cap = carry_cap + chunk_bytes;
+    const size_t idsz = (size_t)h->cfg.id_dtype;
+    for (auto &s : r.slots) {
+        CU(cudaMalloc(&s.d_buf, (size_t)cap + 256));
+        CU(cudaMalloc(&s.d_recoff, (size_t)(max_rows + 2) * sizeof(int64_t)));
+        CU(cudaHostAlloc(&s.h_recoff, (size_t)(max_rows + 2) * sizeof(int64_t), cudaHostAllocDefault));
+        CU(cudaMalloc(&s.d_ids, (size_t)cap * idsz));
+        CU(cudaMalloc(&s.d_out_off, (size_t)(max_rows + 2) * sizeof(int64_t)));
+        if (h->cfg.seq_len > 0) {
+            CU(cudaMalloc(&s.d_batch, (size_t)max_rows * h->cfg.seq_len * sizeof(int32_t)));
+            CU(cudaMalloc(&s.d_mask, (size_t)max_rows * h->cfg.seq_len));
+        }
+        CU(cudaEventCreateWithFlags(&s.ev_h2d, cudaEventDisableTiming));
+        CU(cudaEventCreateWithFlags(&s.ev_carry, cudaEventDisableTiming));
+        CU(cudaEventCreateWithFlags(&s.ev_done, cudaEventDisableTiming));
+        CU(cudaEventCreateWithFlags(&s.ev_off, cudaEventDisableTiming));
+        int rc = ctx_init(h, s.ctx); if (rc) return rc;
+    }
+    return DNATOK_OK;
+}
+
+}  // namespace
+
+// ======================================================================================
+extern "C" {
+
+const char *dnatok_version(void) { return "dnatok-b200 0.1 (sm_100a)"; }
+
+void dnatok_config_default(dnatok_config *cfg, int32_t mode, int32_t k) {
+    memset(cfg, 0, sizeof *cfg);
+    cfg->struct_size = sizeof *cfg;
+    cfg->mode = mode; cfg->k = k; cfg->id_dtype = DNATOK_I32;
+    default_lut(cfg->class_lut);
+    cfg->strip_headers = 1; cfg->pad_id = 0; cfg->unk_id = 1;
+    for (int i = 0; i < 5; ++i) cfg->nt_ids[i] = 2 + i;
+    cfg->base_id = 3; cfg->n_id = 2; cfg->tail_policy = DNATOK_TAIL_PER_BASE;
+    cfg->pad_side = DNATOK_PAD_LEFT; cfg->max_record_bytes = 1 << 20;
+}
+
+int dnatok_create(const dnatok_config *cfg_in, int device, dnatok_t **out) {
+    if (!cfg_in || !out || cfg_in->struct_size != sizeof(dnatok_config)) return DNATOK_EINVAL;
+    *out = nullptr;
+    dnatok_config cfg = *cfg_in;
+    bool zero = true;
+    for (int b = 0; b < 256; ++b) zero = zero && cfg.class_lut[b] == 0;
+    if (zero) default_lut(cfg.class_lut);
+    for (int b = 0; b < 256; ++b)
+        if (cfg.class_lut[b] > DNATOK_CLS_UNK && cfg.class_lut[b] != DNATOK_CLS_SKIP) return DNATOK_EINVAL;
+    if (cfg.strip_headers && cfg.class_lut['\n'] != DNATOK_CLS_SKIP) return DNATOK_EINVAL;
+    if (cfg.mode < DNATOK_SINGLE_NT || cfg.mode > DNATOK_BPE) return DNATOK_EINVAL;
+    if (cfg.id_dtype != DNATOK_I16 && cfg.id_dtype != DNATOK_I32) return DNATOK_EINVAL;
+    if (cfg.seq_len < 0 || (cfg.pad_side != DNATOK_PAD_LEFT && cfg.pad_side != DNATOK_PAD_RIGHT)) return DNATOK_EINVAL;
+    if (cfg.max_record_bytes <= 0) cfg.max_record_bytes = 1 << 20;
+    int64_t max_id = std::max<int64_t>(cfg.unk_id, cfg.pad_id);
+    if (cfg.mode == DNATOK_SINGLE_NT) {
+        for (int i = 0; i < 5; ++i) max_id = std::max<int64_t>(max_id, cfg.nt_ids[i]);
+    } else if (cfg.mode == DNATOK_KMER) {
+        if (cfg.k < 1 || cfg.k > DNATOK_MAX_K) return DNATOK_EINVAL;
+        if (cfg.tail_policy < DNATOK_TAIL_PER_BASE || cfg.tail_policy > DNATOK_TAIL_UNK) return DNATOK_EINVAL;
+        int64_t fk = 1ll << (2 * cfg.k);
+        max_id = std::max<int64_t>(max_id, cfg.base_id + fk - 1 + (cfg.tail_policy == DNATOK_TAIL_PER_BASE ? 5 : 0));
+        if (max_id > 0x7fffffffll) return DNATOK_EINVAL;
+    } else {
+        if (cfg.n_merges < 0 || cfg.n_merges > 65000 || (cfg.n_merges > 0 && !cfg.merges)) return DNATOK_EINVAL;
+        max_id = std::max<int64_t>(max_id, std::max<int64_t>(cfg.n_id, cfg.base_id + 3 + cfg.n_merges));
+    }
+    if (cfg.id_dtype == DNATOK_I16 && max_id > 0x7fff) return DNATOK_EINVAL;
+
+    // BPE rule table (validated before any device work; Q12)
+    std::vector<uint64_t> table;
+    uint32_t mask = 0;
+    if (cfg.mode == DNATOK_BPE) {
+        uint32_t size = 16;
+        while (size < 2u * (uint32_t)cfg.n_merges + 1u) size <<= 1;
+        mask = size - 1;
+        table.assign(size, ~0ull);
+        for (int32_t r = 0; r < cfg.n_merges; ++r) {
+            int32_t L = cfg.merges[2 * r], R = cfg.merges[2 * r + 1];
+            if (L < 0 || R < 0 || L >= 4 + r || R >= 4 + r) return DNATOK_EINVAL;
+            uint32_t key = ((uint32_t)L << 16) | (uint32_t)R, hsh = host_hash(key) & mask;
+            while (table[hsh] != ~0ull) {
+                if ((uint32_t)(table[hsh] >> 32) == key) return DNATOK_EINVAL;   // duplicate pair
+                hsh = (hsh + 1) & mask;
+            }
+            table[hsh] = ((uint64_t)key << 32) | (uint32_t)r;
+        }
+    }
+
+    dnatok_t *h = new (std::nothrow) dnatok();
+    if (!h) return DNATOK_ENOMEM;
+    h->cfg = cfg; h->cfg.merges = nullptr; h->device = device;
+    auto bail = [&](int code) { dnatok_destroy(h); return code; };
+    if (cudaSetDevice(device) != cudaSuccess) return bail(DNATOK_ECUDA);
+    cudaDeviceProp prop;
+    if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) return bail(DNATOK_ECUDA);
+    h->sm_count = prop.multiProcessorCount;
+
+    EncParams &p = h->prm;
+    p.mode = cfg.mode == DNATOK_KMER ? MODE_KMER : MODE_SINGLE_NT;
+    p.k = cfg.mode == DNATOK_KMER ? cfg.k : 1;
+    p.tail_policy = cfg.tail_policy; p.strip_headers = cfg.strip_headers;
+    p.unk_id = cfg.unk_id; p.base_id = cfg.base_id;
+    for (int i = 0; i < 5; ++i) p.nt_ids[i] = cfg.nt_ids[i];
+    p.four_k = cfg.mode == DNATOK_KMER ? (int32_t)(1ll << (2 * cfg.k)) : 0;
+
+    if (cudaMalloc(&h->d_lut, 256) != cudaSuccess) return bail(DNATOK_ENOMEM);
+    if (cudaMemcpy(h->d_lut, cfg.class_lut, 256, cudaMemcpyHostToDevice) != cudaSuccess) return bail(DNATOK_ECUDA);
+    if (cfg.mode == DNATOK_BPE) {
+        h->table_mask = mask;
+        if (cudaMalloc(&h->d_table, table.size() * sizeof(uint64_t)) != cudaSuccess) return bail(DNATOK_ENOMEM);
+        if (cudaMemcpy(h->d_table, table.data(), table.size() * sizeof(uint64_t), cudaMemcpyHostToDevice) != cudaSuccess)
+            return bail(DNATOK_ECUDA);
+        int cap = 256;
+        while (cap < cfg.max_record_bytes && cap < 8192) cap <<= 1;
+        h->bpe_cap = cap;
+        if (cudaFuncSetAttribute(bpe_reads_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                 (int)bpe_smem_bytes(cap)) != cudaSuccess) return bail(DNATOK_ECUDA);
+        int nb = 0;
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, bpe_reads_kernel, BPE_NT, bpe_smem_bytes(cap));
+        h->bpe_ctas_per_sm = std::max(nb, 1);
+    }
+    {
+        int nb = 0;
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, encode_tiles_kernel<int32_t>, NT, sizeof(TileSmem));
+        h->enc_ctas_per_sm = std::max(nb, 1);
+    }
+    if (ctx_init(h, h->ctx) != DNATOK_OK) return bail(DNATOK_ECUDA);
+    *out = h;
+    return DNATOK_OK;
+}
+
+int dnatok_destroy(dnatok_t *h) {
+    if (!h) return DNATOK_OK;
+    cudaSetDevice(h->device);
+    cudaDeviceSynchronize();
+    ring_free(h->ring);
+    ctx_free(h->ctx);
+    cudaFree(h->d_lut); cudaFree(h->d_table);
+    delete h;
+    return DNATOK_OK;
+}
+
+int dnatok_encode(dnatok_t *h, const uint8_t *d_bytes, int64_t n_bytes, const int64_t *d_rec_offsets,
+                  int64_t n_records, void *d_ids_out, int64_t ids_capacity, int64_t *d_out_offsets, void *stream) {
+    if (!h) return DNATOK_EINVAL;
+    if (n_bytes < 0 || n_records < 0 || ids_capacity < 0 || !d_rec_offsets || !d_out_offsets ||
+        (n_bytes > 0 && !d_bytes) || (ids_capacity > 0 && !d_ids_out))
+        return fail(h, DNATOK_EINVAL, "dnatok_encode: bad argument");
+    CU(cudaSetDevice(h->device));
+    return encode_on(h, h->ctx, d_bytes, n_bytes, d_rec_offsets, n_records, 0, d_ids_out, ids_capacity,
+                     d_out_offsets, (cudaStream_t)stream);
+}
+
+int dnatok_pad(dnatok_t *h, const void *d_ids, const int64_t *d_out_offsets, int64_t n_records,
+               int32_t *d_batch_ids, uint8_t *d_mask, void *stream) {
+    if (!h) return DNATOK_EINVAL;
+    if (h->cfg.seq_len <= 0) return fail(h, DNATOK_EINVAL, "dnatok_pad: handle was created with seq_len == 0");
+    if (n_records < 0 || !d_out_offsets || (n_records > 0 && !d_batch_ids))
+        return fail(h, DNATOK_EINVAL, "dnatok_pad: bad argument");
+    CU(cudaSetDevice(h->device));
+    return pad_on(h, d_ids, d_out_offsets, n_records, d_batch_ids, d_mask, (cudaStream_t)stream);
+}
+
+int dnatok_stream_encode(dnatok_t *h, const uint8_t *h_pinned, int64_t n_bytes, const int64_t *h_rec_offsets,
+                         int64_t n_records, int64_t chunk_bytes, int n_streams, int64_t max_rows_per_chunk,
+                         dnatok_batch_fn on_batch, void *user) {
+    if (!h) return DNATOK_EINVAL;
+    if (n_bytes < 0 || n_records < 0 || !h_rec_offsets || chunk_bytes <= 0 || n_streams < 1 || n_streams > 64 ||
+        (n_bytes > 0 && !h_pinned))
+        return fail(h, DNATOK_EINVAL, "dnatok_stream_encode: bad argument");
+    CU(cudaSetDevice(h->device));
+    if (n_bytes > 0) {
+        cudaPointerAttributes at;
+        cudaError_t e = cudaPointerGetAttributes(&at, h_pinned);
+        if (e != cudaSuccess || at.type != cudaMemoryTypeHost) {
+            cudaGetLastError();
+            return fail(h, DNATOK_EINVAL, "dnatok_stream_encode: h_pinned is not page-locked host memory");
+        }
+    }
+    if (max_rows_per_chunk <= 0) max_rows_per_chunk = chunk_bytes / 64 + 2;
+    int rc = ring_setup(h, chunk_bytes, n_streams, max_rows_per_chunk);
+    if (rc) return rc;
+    StreamRing &R = h->ring;
+    const int64_t C = chunk_bytes;
+    const int64_t n_chunks = std::max<int64_t>(1, (n_bytes + C - 1) / C);
+    const size_t idsz = (size_t)h->cfg.id_dtype;
+    int64_t ra = 0;                                   // first record not yet delivered
+    for (int64_t i = 0; i < n_chunks; ++i) {
+        StreamSlot &S = R.slots[i % R.n_slots];
+        cudaStream_t st = R.streams[i % R.n_streams];
+        const int64_t c0 = i * C, c1 = std::min(n_bytes, c0 + C);
+        // records that end in this chunk: h_rec_offsets[r + 1] in (c0, c1] (all the rest in the last chunk)
+        int64_t rb;
+        if (i == n_chunks - 1) rb = n_records;
+        else rb = std::upper_bound(h_rec_offsets + ra + 1, h_rec_offsets + n_records + 1, c1) - h_rec_offsets - 1;
+        if (rb < ra) rb = ra;
+        const int64_t rows = rb - ra;
+        if (rows > R.max_rows) {
+            for (auto s2 : R.streams) cudaStreamSynchronize(s2);
+            return fail(h, DNATOK_ECAPACITY, "chunk %lld holds %lld records > max_rows_per_chunk %lld",
+                        (long long)i, (long long)rows, (long long)R.max_rows);
+        }
+        // bytes of the record cut by the previous boundary live in the previous slot's buffer
+        const int64_t data0 = std::min(h_rec_offsets[ra], c0);       // host offset of the first byte needed
+        const int64_t carry = c0 - data0;
+        if (carry > R.carry_cap) {
+            for (auto s2 : R.streams) cudaStreamSynchronize(s2);
+            return fail(h, DNATOK_ECAPACITY, "record %lld needs %lld carried bytes > max_record_bytes %lld",
+                        (long long)ra, (long long)carry, (long long)R.carry_cap);
+        }
+        uint8_t *d_chunk = S.d_buf + R.carry_cap;
+        // this buffer was last used by chunk i - n_slots (same stream only if n_slots == n_streams) and read by
+        // chunk i - n_slots + 1's carry copy
+        if (i >= R.n_slots) {
+            CU(cudaStreamWaitEvent(st, S.ev_done, 0));
+            CU(cudaStreamWaitEvent(st, R.slots[(i + 1) % R.n_slots].ev_carry, 0));
+        }
+        if (carry > 0) {
+            StreamSlot &Pv = R.slots[(i - 1) % R.n_slots];
+            CU(cudaStreamWaitEvent(st, Pv.ev_h2d, 0));
+            CU(cudaMemcpyAsync(d_chunk - carry, Pv.d_buf + R.carry_cap + (data0 - (c0 - C)), (size_t)carry,
+                               cudaMemcpyDeviceToDevice, st));
+        }
+        CU(cudaEventRecord(S.ev_carry, st));
+        if (c1 > c0) CU(cudaMemcpyAsync(d_chunk, h_pinned + c0, (size_t)(c1 - c0), cudaMemcpyHostToDevice, st));
+        CU(cudaEventRecord(S.ev_h2d, st));
+        // record offsets of this batch (staged through the slot's pinned buffer)
+        CU(cudaEventSynchronize(S.ev_off));
+        memcpy(S.h_recoff, h_rec_offsets + ra, (size_t)(rows + 1) * sizeof(int64_t));
+        CU(cudaMemcpyAsync(S.d_recoff, S.h_recoff, (size_t)(rows + 1) * sizeof(int64_t), cudaMemcpyHostToDevice, st));
+        CU(cudaEventRecord(S.ev_off, st));
+        // encode the whole records [ra, rb): buffer starts at host offset data0
+        const int64_t nb = std::max<int64_t>(0, (rows > 0 ? h_rec_offsets[rb] : data0) - data0);
+        rc = encode_on(h, S.ctx, d_chunk - carry, nb, S.d_recoff, rows, data0, S.d_ids, R.carry_cap + C,
+                       S.d_out_off, st);
+        if (rc) return rc;
+        if (h->cfg.seq_len > 0) {
+            rc = pad_on(h, S.d_ids, S.d_out_off, rows, S.d_batch, S.d_mask, st);
+            if (rc) return rc;
+        }
+        if (on_batch) {
+            dnatok_batch b;
+            b.first_record = ra; b.n_records = rows; b.d_ids = S.d_ids; b.d_out_offsets = S.d_out_off;
+            b.d_batch_ids = h->cfg.seq_len > 0 ? S.d_batch : nullptr;
+            b.d_mask = h->cfg.seq_len > 0 ? S.d_mask : nullptr;
+            b.chunk_index = i; b.stream = (void *)st;
+            on_batch(user, &b);
+        }
+        CU(cudaEventRecord(S.ev_done, st));
+        ra = rb;
+    }
+    (void)idsz;
+    for (auto st : R.streams) CU(cudaStreamSynchronize(st));
+    for (auto &s : R.slots) { rc = status_of(h, s.ctx); if (rc) return rc; }
+    return DNATOK_OK;
+}
+
+int dnatok_check(dnatok_t *h, void *stream) {
+    if (!h) return DNATOK_EINVAL;
+    CU(cudaSetDevice(h->device));
+    CU(cudaStreamSynchronize((cudaStream_t)stream));
+    return status_of(h, h->ctx);
+}
+
+const char *dnatok_last_error(const dnatok_t *h) { return h ? h->err.c_str() : "null handle"; }
+
+int64_t dnatok_launch_count(const dnatok_t *h) { return h ? h->launches : 0; }
+
+}  // extern "C"
