@@ -71,6 +71,7 @@ __device__ __forceinline__ int64_t warp_lower_bound(const EncArgs &A, int64_t lo
         int64_t idx = lo + (int64_t)(lane + 1) * step - 1;
         bool ge = (idx >= hi) ? true : (rec_pos(A, idx) >= pos);
         uint32_t b = __ballot_sync(0xffffffffu, ge);
+        if (!b) return hi;                       // lane 31 probed hi-1 and even that is < pos
         int f = __ffs(b) - 1;                    // first probe that is >= pos (lane 31 probes >= hi-1 or beyond)
         int64_t nlo = lo + (int64_t)f * step;    // everything before probe f-1 (inclusive) is < pos
         int64_t nhi = lo + (int64_t)(f + 1) * step - 1;
@@ -80,7 +81,7 @@ __device__ __forceinline__ int64_t warp_lower_bound(const EncArgs &A, int64_t lo
     int64_t idx = lo + lane;
     bool ge = (idx >= hi) ? true : (rec_pos(A, idx) >= pos);
     uint32_t b = __ballot_sync(0xffffffffu, ge);
-    return lo + (__ffs(b) - 1);
+    return b ? lo + (__ffs(b) - 1) : hi;         // hi - lo == 32: no lane probed hi itself
 }
 
 __device__ __forceinline__ int kept_before(const TileSmem &sm, int p) {   // kept bases at tile positions < p

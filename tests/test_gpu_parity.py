@@ -140,6 +140,16 @@ def test_many_tiny_records_in_one_tile():
         check(data, offs, **kw)
 
 
+@pytest.mark.parametrize("n_rec", [31, 32, 33, 63, 127, 128, 1023, 1024, 4095, 4096, 4097])
+def test_record_counts_around_the_search_fanout(n_rec):
+    # the per-tile record search is 32-ary: counts where a narrowed range is a multiple of 32 hit its edge cases
+    rng = np.random.default_rng(n_rec)
+    lens = rng.integers(250, 350, size=n_rec)
+    data = rng.choice(np.frombuffer(b"ACGTN", dtype=np.uint8), size=int(lens.sum()), p=[.245, .245, .245, .245, .02])
+    offs = np.concatenate([[0], np.cumsum(lens)])
+    check(data, offs, mode="kmer", k=6)
+
+
 def test_records_aligned_to_tile_boundaries():
     rng = np.random.default_rng(6)
     data = rng.choice(np.frombuffer(b"ACGT", dtype=np.uint8), size=8192 * 5)
