@@ -69,6 +69,7 @@ struct EncParams {
     int32_t unk_id, base_id;
     int32_t nt_ids[5];
     int32_t four_k;         // 4^k (KMER; fits: k <= 15)
+    int32_t fast_lut;       // class_lut maps ACGTacgt to 0..3 like the default: arithmetic classification is exact for them
 };
 
 struct EncArgs {

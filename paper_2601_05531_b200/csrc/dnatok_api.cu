@@ -14,7 +14,7 @@
 
 #include "bpe_kernel.cuh"
 #include "common.cuh"
-#include "encode_kernel.cuh"
+#include "encode_v2.cuh"
 #include "pad_kernel.cuh"
 
 using namespace dtk;
@@ -147,7 +147,7 @@ int launch_tiles(dnatok_t *h, EncCtx &c, const EncParams &prm, const uint8_t *d_
     a.mis = (int64_t)(addr & 15);
     a.bytes_al = reinterpret_cast<const uint8_t *>(addr - (uintptr_t)a.mis);
     a.p_end = a.mis + n_bytes;
-    int64_t n_tiles = a.p_end / TB + 1;
+    int64_t n_tiles = a.p_end / TB2 + 1;
     if (n_tiles > 0x7fffffff) return fail(h, DNATOK_EINVAL, "n_bytes too large for one call");
     int rc = ctx_reserve_tiles(h, c, n_tiles, st); if (rc) return rc;
     rc = ctx_next_gen(h, c, st); if (rc) return rc;
@@ -156,7 +156,7 @@ int launch_tiles(dnatok_t *h, EncCtx &c, const EncParams &prm, const uint8_t *d_
     a.lut = h->d_lut; a.descs = c.descs; a.ticket = c.ticket; a.ticket_base = c.ticket_base;
     a.status = c.d_status; a.gen = c.gen; a.n_tiles = (int32_t)n_tiles; a.prm = prm;
     int grid = (int)std::min<int64_t>(n_tiles, (int64_t)h->sm_count * h->enc_ctas_per_sm);
-    encode_tiles_kernel<IdT><<<grid, NT, sizeof(TileSmem), st>>>(a);
+    encode_tiles_v2<IdT><<<grid, NT, sizeof(Smem2), st>>>(a);
     CU(cudaGetLastError());
     c.ticket_base += (unsigned long long)n_tiles + (unsigned long long)grid;
     h->launches += 1;
@@ -380,6 +380,9 @@ int dnatok_create(const dnatok_config *cfg_in, int device, dnatok_t **out) {
     p.unk_id = cfg.unk_id; p.base_id = cfg.base_id;
     for (int i = 0; i < 5; ++i) p.nt_ids[i] = cfg.nt_ids[i];
     p.four_k = cfg.mode == DNATOK_KMER ? (int32_t)(1ll << (2 * cfg.k)) : 0;
+    p.fast_lut = 1;
+    for (int i = 0; i < 4; ++i)
+        if (cfg.class_lut[(uint8_t)"ACGT"[i]] != i || cfg.class_lut[(uint8_t)"acgt"[i]] != i) p.fast_lut = 0;
 
     if (cudaMalloc(&h->d_lut, 256) != cudaSuccess) return bail(DNATOK_ENOMEM);
     if (cudaMemcpy(h->d_lut, cfg.class_lut, 256, cudaMemcpyHostToDevice) != cudaSuccess) return bail(DNATOK_ECUDA);
@@ -399,7 +402,7 @@ int dnatok_create(const dnatok_config *cfg_in, int device, dnatok_t **out) {
     }
     {
         int nb = 0;
-        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, encode_tiles_kernel<int32_t>, NT, sizeof(TileSmem));
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, encode_tiles_v2<int32_t>, NT, sizeof(Smem2));
         h->enc_ctas_per_sm = std::max(nb, 1);
     }
     if (ctx_init(h, h->ctx) != DNATOK_OK) return bail(DNATOK_ECUDA);
