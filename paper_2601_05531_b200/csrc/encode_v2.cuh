@@ -56,12 +56,6 @@ __device__ __forceinline__ unsigned long long from_pos(int q) { return q >= 64 ?
 __device__ __forceinline__ int first_pos(unsigned long long m) { return m ? __clzll((long long)m) : 64; }
 __device__ __forceinline__ int last_pos(unsigned long long m) { return 63 - (__ffsll((long long)m) - 1); }   // m != 0
 
-__device__ __forceinline__ uint32_t ld_relaxed(const uint32_t *p) {
-    uint32_t v;
-    asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
-    return v;
-}
-
 // exclusive block scan of one int per thread (two barriers)
 __device__ __forceinline__ int block_exscan2(int v, Smem2 &sm, int &total) {
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -449,7 +443,7 @@ __global__ void __launch_bounds__(NT) encode_tiles_v2(const __grid_constant__ En
                     t_x = g_hr ? g_x : (t_x == LS_LINE_START ? g_x : t_x);
                     t_hr |= g_hr;
                 }
-                st_release(&D.l_word, (gen << 8) | (t_hr << 2) | t_x);
+                st_vol32(&D.l_word, (gen << 8) | (t_hr << 2) | t_x);
                 sm.ls_in = (t_hr << 2) | t_x;                // parked for warp 0 below
             }
             __syncthreads();
@@ -468,9 +462,9 @@ __global__ void __launch_bounds__(NT) encode_tiles_v2(const __grid_constant__ En
                         const TileDesc &Dj = A.descs[j];
                         int spins = 0;
                         for (;;) {
-                            uint32_t a = ld_acquire(&Dj.l_incl);
+                            uint32_t a = ld_vol32(&Dj.l_incl);
                             if ((a >> 8) == gen) { val = a & 3u; term = true; break; }
-                            a = ld_acquire(&Dj.l_word);
+                            a = ld_vol32(&Dj.l_word);
                             if ((a >> 8) == gen) { val = a & 3u; term = (a >> 2) & 1u; break; }
                             if (++spins > SPIN_LIMIT) { ok = false; break; }
                         }
@@ -494,7 +488,7 @@ __global__ void __launch_bounds__(NT) encode_tiles_v2(const __grid_constant__ En
                 if (lane == 0) {
                     const uint32_t t_hr = mine >> 2, t_x = mine & 3u;
                     const uint32_t ex = t_hr ? t_x : (state == LS_LINE_START ? t_x : state);
-                    st_release(&D.l_incl, (gen << 8) | ex);
+                    st_vol32(&D.l_incl, (gen << 8) | ex);
                     sm.ls_in = state;
                 }
             }
@@ -604,85 +598,99 @@ __global__ void __launch_bounds__(NT) encode_tiles_v2(const __grid_constant__ En
             for (int e = tid; e < m - 1; e += NT) {
                 int ka = kept_before2(sm, (int)(rec_pos2(A, r_lo + e) - t0));
                 int kb = kept_before2(sm, (int)(rec_pos2(A, r_lo + e + 1) - t0));
-                closed_part += (int)tok_count(kb - ka, P);
+                closed_part += tok_count32(kb - ka, P);
             }
         }
         int closed_tokens = 0;
         if (m > 1) (void)block_exscan2(closed_part, sm, closed_tokens);
         if (warp == 0) {
+            const uint32_t tagA = (gen << 2) | ST_AGG, tagI = (gen << 2) | ST_INCL;
+            const int k = P.k;
             Agg G;
-            G.first_kept = first_kept; G.last_kept = last_kept; G.closed_tokens = closed_tokens; G.has_event = m > 0;
-            const uint32_t tn = (uint32_t)min(P.k - 1, last_kept);
+            G.first = qr_of(first_kept, k); G.last = qr_of(last_kept, k); G.closed = closed_tokens; G.has_event = m > 0;
+            const uint32_t tn = (uint32_t)min(k - 1, last_kept);
             uint64_t tl = 0;
             if (lane == 0) for (uint32_t i = 0; i < tn; ++i) tl = (tl << 4) | class_at(sm, PEND + ktot - (int)tn + (int)i);
+            tl = __shfl_sync(0xffffffffu, tl, 0);
             G.tail = tl; G.tail_cnt = tn;
-            Prefix X; X.T = 0; X.open_n = 0; X.tail = 0; X.tail_cnt = 0;
+            Prefix X; X.T = 0; X.open.q = 0; X.open.r = 0; X.tail = 0; X.tail_cnt = 0;
             if (tile > 0) {
                 if (lane == 0) {
-                    D.has_event = G.has_event; D.first_kept = first_kept; D.last_kept = last_kept;
-                    D.closed_tokens = closed_tokens; D.tail = tl; D.tail_cnt = tn;
-                    st_release(&D.status, (gen << 2) | ST_AGG);
+                    st_vol128(&D.a0, make_uint4(tagA, (uint32_t)first_kept, (uint32_t)last_kept, (uint32_t)closed_tokens));
+                    st_vol128(&D.a1, make_uint4(tagA, tn | ((uint32_t)(m > 0) << 8), (uint32_t)tl, (uint32_t)(tl >> 32)));
                 }
-                // warp-parallel look-back: lane l inspects tile base - l
+                // warp-parallel look-back: lane l inspects tile base - l; one round trip per 32 tiles
                 Agg acc; bool have = false, ok = true, done = false;
                 for (int base = tile - 1; !done && ok; base -= 32) {
                     const int j = base - lane;
                     uint32_t st = ST_INCL;                   // tiles before 0 carry the empty inclusive prefix
+                    Agg Aj; Prefix Xj;
+                    Aj.first.q = Aj.last.q = Aj.closed = 0; Aj.first.r = Aj.last.r = 0; Aj.tail = 0; Aj.tail_cnt = 0; Aj.has_event = 0;
+                    Xj.T = 0; Xj.open.q = 0; Xj.open.r = 0; Xj.tail = 0; Xj.tail_cnt = 0;
                     if (j >= 0) {
                         const TileDesc &Dj = A.descs[j];
                         int spins = 0;
-                        while ((((st = ld_acquire(&Dj.status)) >> 2) != gen || (st & 3u) == ST_EMPTY)) {
+                        for (;;) {
+                            const uint4 w0 = ld_vol128(&Dj.i0), w1 = ld_vol128(&Dj.i1), w2 = ld_vol128(&Dj.i2);
+                            const uint4 a0 = ld_vol128(&Dj.a0), a1 = ld_vol128(&Dj.a1);
+                            if (w0.x == tagI && w1.x == tagI && w2.x == tagI) {
+                                st = ST_INCL;
+                                Xj.T = (int64_t)(((uint64_t)w0.w << 32) | w0.z);
+                                Xj.tail_cnt = w0.y & 0xffu; Xj.open.r = (int32_t)(w0.y >> 8);
+                                Xj.open.q = (int64_t)(((uint64_t)w1.w << 32) | w1.z);
+                                Xj.tail = ((uint64_t)w2.w << 32) | w2.z;
+                                break;
+                            }
+                            if (a0.x == tagA && a1.x == tagA) {
+                                st = ST_AGG;
+                                Aj.first = qr_of((int)a0.y, k); Aj.last = qr_of((int)a0.z, k); Aj.closed = (int64_t)a0.w;
+                                Aj.tail_cnt = a1.y & 0xffu; Aj.has_event = a1.y >> 8;
+                                Aj.tail = ((uint64_t)a1.w << 32) | a1.z;
+                                break;
+                            }
                             if (++spins > SPIN_LIMIT) { ok = false; break; }
                         }
-                        st &= 3u;
                     }
                     ok = __all_sync(0xffffffffu, ok);
                     if (!ok) break;
                     const uint32_t ib = __ballot_sync(0xffffffffu, st == ST_INCL);
                     const int f = ib ? __ffs(ib) - 1 : 32;   // nearest tile with an inclusive prefix
-                    // every lane loads what it will contribute
-                    Agg Aj; Prefix Xj;
-                    Aj.first_kept = Aj.last_kept = Aj.closed_tokens = 0; Aj.tail = 0; Aj.tail_cnt = 0; Aj.has_event = 0;
-                    Xj.T = 0; Xj.open_n = 0; Xj.tail = 0; Xj.tail_cnt = 0;
-                    if (j >= 0) {
-                        const TileDesc &Dj = A.descs[j];
-                        if (lane == f) { Xj.T = Dj.T; Xj.open_n = Dj.open_n; Xj.tail = Dj.ptail; Xj.tail_cnt = Dj.ptail_cnt; }
-                        else if (lane < f) {
-                            Aj.first_kept = Dj.first_kept; Aj.last_kept = Dj.last_kept; Aj.closed_tokens = Dj.closed_tokens;
-                            Aj.tail = Dj.tail; Aj.tail_cnt = Dj.tail_cnt; Aj.has_event = Dj.has_event;
-                        }
+                    if (lane >= f) {                         // identity element beyond the nearest inclusive prefix
+                        Aj.first.q = Aj.last.q = Aj.closed = 0; Aj.first.r = Aj.last.r = 0; Aj.tail = 0; Aj.tail_cnt = 0; Aj.has_event = 0;
                     }
-                    // fold lanes f-1 .. 0 (far to near) in front of what nearer rounds already composed
-                    const int top = (f < 32 ? f : 32) - 1;
-                    Agg rnd; bool have_r = false;
-                    for (int l = top; l >= 0; --l) {
-                        Agg B;
-                        B.first_kept = __shfl_sync(0xffffffffu, Aj.first_kept, l);
-                        B.last_kept = __shfl_sync(0xffffffffu, Aj.last_kept, l);
-                        B.closed_tokens = __shfl_sync(0xffffffffu, Aj.closed_tokens, l);
-                        B.tail = __shfl_sync(0xffffffffu, Aj.tail, l);
-                        B.tail_cnt = __shfl_sync(0xffffffffu, Aj.tail_cnt, l);
-                        B.has_event = __shfl_sync(0xffffffffu, Aj.has_event, l);
-                        rnd = have_r ? agg_compose(rnd, B, P) : B;
-                        have_r = true;
+                    // ordered tree reduction: after the step of distance d lane l holds tiles [l, l + 2d) composed far -> near
+#pragma unroll
+                    for (int d = 1; d < 32; d <<= 1) {
+                        Agg B;                               // what lane l + d holds: the farther (earlier) run
+                        B.first.q = __shfl_down_sync(0xffffffffu, Aj.first.q, d);
+                        B.last.q = __shfl_down_sync(0xffffffffu, Aj.last.q, d);
+                        B.closed = __shfl_down_sync(0xffffffffu, Aj.closed, d);
+                        B.tail = __shfl_down_sync(0xffffffffu, Aj.tail, d);
+                        const uint32_t pk = (uint32_t)Aj.first.r | ((uint32_t)Aj.last.r << 4) | (Aj.tail_cnt << 8) | (Aj.has_event << 12);
+                        const uint32_t pb = __shfl_down_sync(0xffffffffu, pk, d);
+                        B.first.r = (int32_t)(pb & 15u); B.last.r = (int32_t)((pb >> 4) & 15u); B.tail_cnt = (pb >> 8) & 15u; B.has_event = pb >> 12;
+                        if (lane + d < 32) Aj = agg_compose(B, Aj, P);
                     }
-                    if (have_r) { acc = have ? agg_compose(rnd, acc, P) : rnd; have = true; }
+                    // lane 0 now holds this round's tiles; put it in front of what nearer rounds composed
+                    if (f > 0) { acc = have ? agg_compose(Aj, acc, P) : Aj; have = true; }
                     if (f < 32) {
-                        X.T = __shfl_sync(0xffffffffu, Xj.T, f); X.open_n = __shfl_sync(0xffffffffu, Xj.open_n, f);
+                        X.T = __shfl_sync(0xffffffffu, Xj.T, f); X.open.q = __shfl_sync(0xffffffffu, Xj.open.q, f);
+                        X.open.r = __shfl_sync(0xffffffffu, Xj.open.r, f);
                         X.tail = __shfl_sync(0xffffffffu, Xj.tail, f); X.tail_cnt = __shfl_sync(0xffffffffu, Xj.tail_cnt, f);
                         done = true;
                     }
                 }
                 if (!ok && lane == 0) A.status[1] = 1u;
-                if (have) X = prefix_apply(X, acc, P);
+                if (have) X = prefix_apply(X, acc, P);       // valid in lane 0
             }
             if (lane == 0) {
                 sm.pin = X;
-                Prefix Y = prefix_apply(X, G, P);
-                D.T = Y.T; D.open_n = Y.open_n; D.ptail = Y.tail; D.ptail_cnt = Y.tail_cnt;
-                st_release(&D.status, (gen << 2) | ST_INCL);
+                const Prefix Y = prefix_apply(X, G, P);
+                st_vol128(&D.i0, make_uint4(tagI, Y.tail_cnt | ((uint32_t)Y.open.r << 8), (uint32_t)Y.T, (uint32_t)((uint64_t)Y.T >> 32)));
+                st_vol128(&D.i1, make_uint4(tagI, 0u, (uint32_t)Y.open.q, (uint32_t)((uint64_t)Y.open.q >> 32)));
+                st_vol128(&D.i2, make_uint4(tagI, 0u, (uint32_t)Y.tail, (uint32_t)(Y.tail >> 32)));
                 // carried bases of the open record go in front of the stream
-                const int pend = (P.mode == MODE_KMER) ? (int)(X.open_n % P.k) : 0;
+                const int pend = (P.mode == MODE_KMER) ? X.open.r : 0;
                 uint32_t cw = 0, bw = 0, nw = 0;
                 for (int i = 0; i < pend; ++i) {
                     const uint32_t c = (uint32_t)((X.tail >> (4 * (pend - 1 - i))) & 0xfu);
@@ -699,13 +707,12 @@ __global__ void __launch_bounds__(NT) encode_tiles_v2(const __grid_constant__ En
 
         // ---- 6. emit ---------------------------------------------------------------------------------------------
         const Prefix X = sm.pin;
-        const int pend = (P.mode == MODE_KMER) ? (int)(X.open_n % P.k) : 0;
-        {   // the record that was open at the tile's start
-            int64_t done = (P.mode == MODE_KMER) ? X.open_n / P.k : X.open_n;
-            emit_segment2<IdT>(A, sm, PEND - pend, pend + first_kept, m > 0, A.out_bias + X.T + done, tid, NT);
+        const int pend = (P.mode == MODE_KMER) ? X.open.r : 0;
+        {   // the record that was open at the tile's start: X.open.q of its windows were emitted by earlier tiles
+            emit_segment2<IdT>(A, sm, PEND - pend, pend + first_kept, m > 0, A.out_bias + X.T + X.open.q, tid, NT);
         }
         if (m > 0) {
-            int64_t base_T = A.out_bias + X.T + tok_count(X.open_n + first_kept, P);   // = out_offsets[r_lo]
+            int64_t base_T = A.out_bias + X.T + qr_tokens(qr_add(X.open, qr_of(first_kept, P.k), P.k), P);   // = out_offsets[r_lo]
             for (int c0 = 0; c0 < m; c0 += EV_CAP) {
                 const int e = c0 + tid, cm = min(EV_CAP, m - c0);
                 int ke = 0, ne = 0, te = 0;
@@ -713,7 +720,7 @@ __global__ void __launch_bounds__(NT) encode_tiles_v2(const __grid_constant__ En
                     ke = kept_before2(sm, (int)(rec_pos2(A, r_lo + e) - t0));
                     int kn = (e + 1 < m) ? kept_before2(sm, (int)(rec_pos2(A, r_lo + e + 1) - t0)) : ktot;
                     ne = kn - ke;
-                    te = (e + 1 < m) ? (int)tok_count(ne, P) : 0;
+                    te = (e + 1 < m) ? tok_count32(ne, P) : 0;
                 }
                 int chunk_total;
                 int ex = block_exscan2(te, sm, chunk_total);
