@@ -329,7 +329,7 @@ def run_ours(args) -> None:
     launches = tok.launch_count - launches0
     tok.check()
     ms_per_step = max_over_ranks(total_ms / args.steps)
-    launches_per_step = (1 if tokkw["mode"] != "bpe" else 4) + (1 if L else 0)   # what one step() enqueues
+    launches_per_step = (2 if tokkw["mode"] != "bpe" else 5) + (1 if L else 0)   # pre-pass + encode (+ BPE passes) (+ pad)
     assert launches >= launches_per_step * args.steps
 
     # ---- parity on sampled records against the oracle (untimed) -----------------------------------
@@ -359,7 +359,7 @@ def run_ours(args) -> None:
     alg_bytes = n_bytes + (n_rec + 1) * 8 + out_bytes + pad_bytes  # bytes + offsets in, ids + CSR offsets out
     kern_ms = float(np.median(per_step_ms))
     roof = {"bound": "hbm" if tokkw["mode"] != "bpe" else "alu",
-            "kernel": "encode_tiles_kernel" if tokkw["mode"] != "bpe" else "bpe_reads_kernel",
+            "kernel": "encode_tiles_v3" if tokkw["mode"] != "bpe" else "bpe_reads_kernel",
             "achieved": alg_bytes / (kern_ms * 1e-3) / 1e9, "peak": peak, "unit": "GB/s",
             "peak_source": peak_src, "algorithmic_bytes_per_launch": alg_bytes,
             "bytes_per_base": alg_bytes / max(1, bases), "kernel_ms": kern_ms,

@@ -14,7 +14,7 @@
 
 #include "bpe_kernel.cuh"
 #include "common.cuh"
-#include "encode_v2.cuh"
+#include "encode_v3.cuh"
 #include "pad_kernel.cuh"
 
 using namespace dtk;
@@ -24,6 +24,7 @@ namespace {
 // scan scratch of one in-flight encode: tile descriptors, ticket counter, host-mapped status words
 struct EncCtx {
     TileDesc *descs = nullptr;
+    int64_t *first_rec = nullptr;      // [descs_cap + 1] record range of every tile (pre-pass output)
     int64_t descs_cap = 0;
     unsigned long long *ticket = nullptr;
     unsigned long long ticket_base = 0;
@@ -113,7 +114,7 @@ int ctx_init(dnatok_t *h, EncCtx &c) {
 }
 
 void ctx_free(EncCtx &c) {
-    cudaFree(c.descs); cudaFree(c.ticket); cudaFreeHost(c.h_status);
+    cudaFree(c.descs); cudaFree(c.first_rec); cudaFree(c.ticket); cudaFreeHost(c.h_status);
     cudaFree(c.cls); cudaFree(c.tmp_tok); cudaFree(c.koff); cudaFree(c.tok_cnt);
     c = EncCtx();
 }
@@ -123,8 +124,10 @@ int ctx_reserve_tiles(dnatok_t *h, EncCtx &c, int64_t n_tiles, cudaStream_t st) 
     if (n_tiles <= c.descs_cap) return DNATOK_OK;
     int64_t cap = std::max<int64_t>(n_tiles + n_tiles / 4, 1024);
     if (c.descs) CU(cudaFreeAsync(c.descs, st));
-    c.descs = nullptr; c.descs_cap = 0;
+    if (c.first_rec) CU(cudaFreeAsync(c.first_rec, st));
+    c.descs = nullptr; c.first_rec = nullptr; c.descs_cap = 0;
     CU(cudaMallocAsync((void **)&c.descs, (size_t)cap * sizeof(TileDesc), st));
+    CU(cudaMallocAsync((void **)&c.first_rec, (size_t)(cap + 1) * sizeof(int64_t), st));
     CU(cudaMemsetAsync(c.descs, 0, (size_t)cap * sizeof(TileDesc), st));
     c.descs_cap = cap;
     return DNATOK_OK;
@@ -147,19 +150,21 @@ int launch_tiles(dnatok_t *h, EncCtx &c, const EncParams &prm, const uint8_t *d_
     a.mis = (int64_t)(addr & 15);
     a.bytes_al = reinterpret_cast<const uint8_t *>(addr - (uintptr_t)a.mis);
     a.p_end = a.mis + n_bytes;
-    int64_t n_tiles = a.p_end / TB2 + 1;
+    int64_t n_tiles = a.p_end / TB + 1;
     if (n_tiles > 0x7fffffff) return fail(h, DNATOK_EINVAL, "n_bytes too large for one call");
     int rc = ctx_reserve_tiles(h, c, n_tiles, st); if (rc) return rc;
     rc = ctx_next_gen(h, c, st); if (rc) return rc;
     a.rec_off = d_rec_off; a.n_rec = n_rec; a.off_bias = off_bias;
     a.ids = ids; a.ids_cap = ids_cap; a.out_off = out_off; a.out_bias = 0;
-    a.lut = h->d_lut; a.descs = c.descs; a.ticket = c.ticket; a.ticket_base = c.ticket_base;
+    a.lut = h->d_lut; a.descs = c.descs; a.first_rec = c.first_rec; a.ticket = c.ticket; a.ticket_base = c.ticket_base;
     a.status = c.d_status; a.gen = c.gen; a.n_tiles = (int32_t)n_tiles; a.prm = prm;
     int grid = (int)std::min<int64_t>(n_tiles, (int64_t)h->sm_count * h->enc_ctas_per_sm);
-    encode_tiles_v2<IdT><<<grid, NT, sizeof(Smem2), st>>>(a);
+    tile_first_rec_kernel<<<(unsigned)((n_tiles + 1 + 255) / 256), 256, 0, st>>>(a);
+    CU(cudaGetLastError());
+    encode_tiles_v3<IdT><<<grid, NT, sizeof(Smem3), st>>>(a);
     CU(cudaGetLastError());
     c.ticket_base += (unsigned long long)n_tiles + (unsigned long long)grid;
-    h->launches += 1;
+    h->launches += 2;
     return DNATOK_OK;
 }
 
@@ -383,6 +388,8 @@ int dnatok_create(const dnatok_config *cfg_in, int device, dnatok_t **out) {
     p.fast_lut = 1;
     for (int i = 0; i < 4; ++i)
         if (cfg.class_lut[(uint8_t)"ACGT"[i]] != i || cfg.class_lut[(uint8_t)"acgt"[i]] != i) p.fast_lut = 0;
+    p.fast_n = cfg.class_lut['N'] == DNATOK_CLS_N && cfg.class_lut['n'] == DNATOK_CLS_N;
+    p.kmagic = p.k >= 2 ? (uint32_t)((1ull << 32) / (uint32_t)p.k) + 1u : 0u;
 
     if (cudaMalloc(&h->d_lut, 256) != cudaSuccess) return bail(DNATOK_ENOMEM);
     if (cudaMemcpy(h->d_lut, cfg.class_lut, 256, cudaMemcpyHostToDevice) != cudaSuccess) return bail(DNATOK_ECUDA);
@@ -402,7 +409,7 @@ int dnatok_create(const dnatok_config *cfg_in, int device, dnatok_t **out) {
     }
     {
         int nb = 0;
-        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, encode_tiles_v2<int32_t>, NT, sizeof(Smem2));
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, encode_tiles_v3<int32_t>, NT, sizeof(Smem3));
         h->enc_ctas_per_sm = std::max(nb, 1);
     }
     if (ctx_init(h, h->ctx) != DNATOK_OK) return bail(DNATOK_ECUDA);
