@@ -289,6 +289,7 @@ def run_ours(args) -> None:
     idsz = int(tokkw.get("id_dtype", 4))
     L = spec["seq_len"]
 
+    dn.SUPER_TILE = args.super_tile
     tok = dn.DNATok(**tokkw, device=local)
     d_bytes = pinned.cuda(non_blocking=True)
     d_off = torch.from_numpy(w.offsets).cuda()
@@ -359,7 +360,7 @@ def run_ours(args) -> None:
     alg_bytes = n_bytes + (n_rec + 1) * 8 + out_bytes + pad_bytes  # bytes + offsets in, ids + CSR offsets out
     kern_ms = float(np.median(per_step_ms))
     roof = {"bound": "hbm" if tokkw["mode"] != "bpe" else "alu",
-            "kernel": "encode_tiles_v3" if tokkw["mode"] != "bpe" else "bpe_reads_kernel",
+            "kernel": "encode_tiles_v4" if tokkw["mode"] != "bpe" else "bpe_reads_kernel",
             "achieved": alg_bytes / (kern_ms * 1e-3) / 1e9, "peak": peak, "unit": "GB/s",
             "peak_source": peak_src, "algorithmic_bytes_per_launch": alg_bytes,
             "bytes_per_base": alg_bytes / max(1, bases), "kernel_ms": kern_ms,
@@ -455,6 +456,7 @@ def main() -> None:
     ap.add_argument("--streams", type=int, default=4)
     ap.add_argument("--traffic", type=float, default=None,
                     help="ncu dram read+write bytes per launch of the dominant kernel (from profiles/)")
+    ap.add_argument("--super-tile", type=int, default=0, help="tuning: sub-tiles per super-tile (0 = automatic)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--no-parity", action="store_true")

@@ -168,6 +168,14 @@ const char *dnatok_last_error(const dnatok_t *h);
 /* Number of kernels this library has launched on the handle since create (bench.py's gpu_launches).    */
 int64_t dnatok_launch_count(const dnatok_t *h);
 
+/*
+ * Tuning knob of the single-pass encoder: the flat byte buffer is cut into super-tiles of
+ * sub_tiles x 16 KiB, the unit of the chained scan.  0 (default) = chosen per call from n_bytes and the SM
+ * count; 1..8 = fixed (tests use this to exercise every size on small inputs).  Results never depend on it.
+ * EINVAL outside 0..8.
+ */
+int dnatok_set_super_tile(dnatok_t *h, int32_t sub_tiles);
+
 /* Library version string, e.g. "dnatok-b200 0.1 (sm_100a)".                                            */
 const char *dnatok_version(void);
 

@@ -19,7 +19,8 @@ enum : int { TAIL_PER_BASE = 0, TAIL_DROP = 1, TAIL_UNK = 2 };
 // ---- tile geometry -------------------------------------------------------------------
 constexpr int NT = 256;                 // threads per CTA
 constexpr int LB = 64;                  // input bytes per thread
-constexpr int TB = NT * LB;             // input bytes per tile (16 KiB)
+constexpr int TB = NT * LB;             // input bytes per sub-tile (16 KiB)
+constexpr int S_MAX = 8;                // sub-tiles per super-tile (the unit of the chained scan), at most
 
 // ---- scan protocol -------------------------------------------------------------------
 enum : uint32_t { ST_EMPTY = 0, ST_AGG = 1, ST_INCL = 2 };
@@ -27,21 +28,22 @@ enum : uint32_t { LS_LINE_START = 0, LS_IN_LINE = 1, LS_IN_HEADER = 2 };
 enum : uint32_t { LK_NONE = 0, LK_SUMMARY = 1, LK_FINAL = 2 };
 constexpr int SPIN_LIMIT = 1 << 22;     // bounded spin: a broken chain sets the status word instead of hanging
 
-// One 64-byte descriptor per tile, made of self-validating words: every 16-byte word carries the tag
+// One 64-byte descriptor per super-tile, made of self-validating words: every 16-byte word carries the tag
 // (generation << 2 | ST_*) of the call that wrote it, is written with one 16-byte store and read with one
 // 16-byte load that bypasses L1, so no fence or acquire/release pair is needed and the scratch never needs
-// clearing between calls.  `a` describes the tile alone (aggregate), i0/i1 the whole prefix up to and
-// including the tile (inclusive).  Class tails hold 3 bits per class, newest class lowest.
-//   a  = { tagA, first_kept | last_kept << 16, closed | has_event << 16 | tail_cnt << 17 | tail_hi10 << 21, tail_lo32 }
+// clearing between calls.  a0/a1 describe the super-tile alone (aggregate), i0/i1 the whole prefix up to and
+// including it (inclusive).  Class tails hold 3 bits per class, newest class lowest.
+//   a0 = { tagA, first_kept, last_kept, closed | has_event << 31 }
+//   a1 = { tagA, tail_cnt | tail_hi10 << 4, tail_lo32, 0 }
 //   i0 = { tagI, T lo, T hi, open_r | tail_cnt << 4 | tail_hi10 << 8 }
 //   i1 = { tagI, open_q lo, open_q hi, tail_lo32 }
-//   ls = gen << 8 | LK_* << 2 | line state          (line-state chain, one 4-byte word)
+// The line-state chain has one 4-byte word per super-tile in an array of its own:
+//   ls = gen << 8 | LK_* << 2 | line state
 struct __align__(16) TileDesc {
-    uint4 a;
+    uint4 a0;
+    uint4 a1;
     uint4 i0;
     uint4 i1;
-    uint32_t ls;
-    uint32_t pad_[3];
 };
 static_assert(sizeof(TileDesc) == 64, "TileDesc layout");
 
@@ -71,13 +73,16 @@ struct EncArgs {
     int64_t *out_off;             // [n_rec + 1]
     int64_t out_bias;             // added to every out_off value and id position (0)
     const uint8_t *lut;           // [256] device
-    TileDesc *descs;
-    int64_t *first_rec;           // [n_tiles + 1]: first r in [0, n_rec] whose position is >= tile * TB (n_rec + 1 if none)
+    TileDesc *descs;              // [n_tiles]
+    uint32_t *ls;                 // [n_tiles] line-state chain words
+    int64_t *first_rec;           // [n_tiles + 1]: first r in [0, n_rec] whose position is >= tile * S * TB (n_rec + 1 if none)
+    int32_t *rec_k;               // [n_rec + 1] scratch: kept bases of the super-tile before each record start (many-starts path)
     unsigned long long *ticket;   // tile ticket counter
     unsigned long long ticket_base;
     uint32_t *status;             // device-mapped host status word
     uint32_t gen;
-    int32_t n_tiles;
+    int32_t n_tiles;              // super-tiles
+    int32_t S;                    // sub-tiles per super-tile (1..S_MAX)
     EncParams prm;
 };
 

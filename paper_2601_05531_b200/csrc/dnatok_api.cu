@@ -1,7 +1,7 @@
 // dnatok_api.cu -- host side of the C-ABI declared in include/dnatok.h.
 //
 // Argument marshalling, scratch management and the pinned multi-stream scheduler; every
-// step of the hot path itself runs in the kernels of encode_kernel.cuh / bpe_kernel.cuh /
+// step of the hot path itself runs in the kernels of encode_v4.cuh / bpe_kernel.cuh /
 // pad_kernel.cuh.  There is no CPU fallback anywhere in this file.
 #include "../../include/dnatok.h"
 
@@ -14,7 +14,7 @@
 
 #include "bpe_kernel.cuh"
 #include "common.cuh"
-#include "encode_v3.cuh"
+#include "encode_v4.cuh"
 #include "pad_kernel.cuh"
 
 using namespace dtk;
@@ -24,8 +24,11 @@ namespace {
 // scan scratch of one in-flight encode: tile descriptors, ticket counter, host-mapped status words
 struct EncCtx {
     TileDesc *descs = nullptr;
-    int64_t *first_rec = nullptr;      // [descs_cap + 1] record range of every tile (pre-pass output)
+    uint32_t *ls = nullptr;            // [descs_cap] line-state chain words
+    int64_t *first_rec = nullptr;      // [descs_cap + 1] record range of every super-tile (pre-pass output)
     int64_t descs_cap = 0;
+    int32_t *rec_k = nullptr;          // [reck_cap] kept-base index of every record start (many-starts path)
+    int64_t reck_cap = 0;
     unsigned long long *ticket = nullptr;
     unsigned long long ticket_base = 0;
     uint32_t *h_status = nullptr;      // pinned + mapped: [0] capacity overflow, [1] scan protocol failure
@@ -69,6 +72,7 @@ struct dnatok {
     EncCtx ctx;
     StreamRing ring;
     int enc_ctas_per_sm = 1, bpe_ctas_per_sm = 1;
+    int force_S = 0;                   // dnatok_set_super_tile: fixed super-tile size in sub-tiles (0 = automatic)
     int64_t launches = 0;
     std::string err;
 };
@@ -114,21 +118,31 @@ int ctx_init(dnatok_t *h, EncCtx &c) {
 }
 
 void ctx_free(EncCtx &c) {
-    cudaFree(c.descs); cudaFree(c.first_rec); cudaFree(c.ticket); cudaFreeHost(c.h_status);
+    cudaFree(c.descs); cudaFree(c.ls); cudaFree(c.first_rec); cudaFree(c.rec_k); cudaFree(c.ticket); cudaFreeHost(c.h_status);
     cudaFree(c.cls); cudaFree(c.tmp_tok); cudaFree(c.koff); cudaFree(c.tok_cnt);
     c = EncCtx();
 }
 
 // stream-ordered growth of the tile-descriptor array (never synchronises the host)
-int ctx_reserve_tiles(dnatok_t *h, EncCtx &c, int64_t n_tiles, cudaStream_t st) {
+int ctx_reserve_tiles(dnatok_t *h, EncCtx &c, int64_t n_tiles, int64_t n_rec, cudaStream_t st) {
+    if (n_rec + 1 > c.reck_cap) {
+        int64_t cap = std::max<int64_t>(n_rec + 1 + n_rec / 4, 1024);
+        if (c.rec_k) CU(cudaFreeAsync(c.rec_k, st));
+        c.rec_k = nullptr; c.reck_cap = 0;
+        CU(cudaMallocAsync((void **)&c.rec_k, (size_t)cap * sizeof(int32_t), st));
+        c.reck_cap = cap;
+    }
     if (n_tiles <= c.descs_cap) return DNATOK_OK;
     int64_t cap = std::max<int64_t>(n_tiles + n_tiles / 4, 1024);
     if (c.descs) CU(cudaFreeAsync(c.descs, st));
+    if (c.ls) CU(cudaFreeAsync(c.ls, st));
     if (c.first_rec) CU(cudaFreeAsync(c.first_rec, st));
-    c.descs = nullptr; c.first_rec = nullptr; c.descs_cap = 0;
+    c.descs = nullptr; c.ls = nullptr; c.first_rec = nullptr; c.descs_cap = 0;
     CU(cudaMallocAsync((void **)&c.descs, (size_t)cap * sizeof(TileDesc), st));
+    CU(cudaMallocAsync((void **)&c.ls, (size_t)cap * sizeof(uint32_t), st));
     CU(cudaMallocAsync((void **)&c.first_rec, (size_t)(cap + 1) * sizeof(int64_t), st));
     CU(cudaMemsetAsync(c.descs, 0, (size_t)cap * sizeof(TileDesc), st));
+    CU(cudaMemsetAsync(c.ls, 0, (size_t)cap * sizeof(uint32_t), st));
     c.descs_cap = cap;
     return DNATOK_OK;
 }
@@ -136,6 +150,7 @@ int ctx_reserve_tiles(dnatok_t *h, EncCtx &c, int64_t n_tiles, cudaStream_t st) 
 int ctx_next_gen(dnatok_t *h, EncCtx &c, cudaStream_t st) {
     if (++c.gen >= (1u << 24) - 1) {       // generation tags are 24 bits wide in TileDesc::l_word
         if (c.descs) CU(cudaMemsetAsync(c.descs, 0, (size_t)c.descs_cap * sizeof(TileDesc), st));
+        if (c.ls) CU(cudaMemsetAsync(c.ls, 0, (size_t)c.descs_cap * sizeof(uint32_t), st));
         c.gen = 1;
     }
     return DNATOK_OK;
@@ -150,18 +165,25 @@ int launch_tiles(dnatok_t *h, EncCtx &c, const EncParams &prm, const uint8_t *d_
     a.mis = (int64_t)(addr & 15);
     a.bytes_al = reinterpret_cast<const uint8_t *>(addr - (uintptr_t)a.mis);
     a.p_end = a.mis + n_bytes;
-    int64_t n_tiles = a.p_end / TB + 1;
+    // super-tile size: the chained scan advances 32 super-tiles per L2 round trip, so large inputs want large S;
+    // small inputs want enough super-tiles to occupy every CTA slot a few times over
+    const int64_t slots = (int64_t)h->sm_count * h->enc_ctas_per_sm;
+    int S = S_MAX;
+    while (S > 1 && a.p_end / ((int64_t)S * TB) + 1 < 3 * slots) S >>= 1;
+    if (h->force_S > 0) S = h->force_S;
+    a.S = S;
+    int64_t n_tiles = a.p_end / ((int64_t)S * TB) + 1;
     if (n_tiles > 0x7fffffff) return fail(h, DNATOK_EINVAL, "n_bytes too large for one call");
-    int rc = ctx_reserve_tiles(h, c, n_tiles, st); if (rc) return rc;
+    int rc = ctx_reserve_tiles(h, c, n_tiles, n_rec, st); if (rc) return rc;
     rc = ctx_next_gen(h, c, st); if (rc) return rc;
     a.rec_off = d_rec_off; a.n_rec = n_rec; a.off_bias = off_bias;
     a.ids = ids; a.ids_cap = ids_cap; a.out_off = out_off; a.out_bias = 0;
-    a.lut = h->d_lut; a.descs = c.descs; a.first_rec = c.first_rec; a.ticket = c.ticket; a.ticket_base = c.ticket_base;
+    a.lut = h->d_lut; a.descs = c.descs; a.ls = c.ls; a.rec_k = c.rec_k; a.first_rec = c.first_rec; a.ticket = c.ticket; a.ticket_base = c.ticket_base;
     a.status = c.d_status; a.gen = c.gen; a.n_tiles = (int32_t)n_tiles; a.prm = prm;
     int grid = (int)std::min<int64_t>(n_tiles, (int64_t)h->sm_count * h->enc_ctas_per_sm);
     tile_first_rec_kernel<<<(unsigned)((n_tiles + 1 + 255) / 256), 256, 0, st>>>(a);
     CU(cudaGetLastError());
-    encode_tiles_v3<IdT><<<grid, NT, sizeof(Smem3), st>>>(a);
+    encode_tiles_v4<IdT><<<grid, NT, sizeof(Smem4), st>>>(a);
     CU(cudaGetLastError());
     c.ticket_base += (unsigned long long)n_tiles + (unsigned long long)grid;
     h->launches += 2;
@@ -408,9 +430,15 @@ int dnatok_create(const dnatok_config *cfg_in, int device, dnatok_t **out) {
         h->bpe_ctas_per_sm = std::max(nb, 1);
     }
     {
+        // the stream of one super-tile needs more than the default 48 KiB of shared memory per CTA
+        if (cudaFuncSetAttribute(encode_tiles_v4<int32_t>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Smem4)) != cudaSuccess ||
+            cudaFuncSetAttribute(encode_tiles_v4<int16_t>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Smem4)) != cudaSuccess ||
+            cudaFuncSetAttribute(encode_tiles_v4<uint8_t>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Smem4)) != cudaSuccess)
+            return bail(DNATOK_ECUDA);
         int nb = 0;
-        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, encode_tiles_v3<int32_t>, NT, sizeof(Smem3));
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, encode_tiles_v4<int32_t>, NT, sizeof(Smem4));
         h->enc_ctas_per_sm = std::max(nb, 1);
+
     }
     if (ctx_init(h, h->ctx) != DNATOK_OK) return bail(DNATOK_ECUDA);
     *out = h;
@@ -548,6 +576,13 @@ int dnatok_check(dnatok_t *h, void *stream) {
     CU(cudaSetDevice(h->device));
     CU(cudaStreamSynchronize((cudaStream_t)stream));
     return status_of(h, h->ctx);
+}
+
+int dnatok_set_super_tile(dnatok_t *h, int32_t sub_tiles) {
+    if (!h) return DNATOK_EINVAL;
+    if (sub_tiles < 0 || sub_tiles > S_MAX) return fail(h, DNATOK_EINVAL, "dnatok_set_super_tile: sub_tiles must be in 0..%d", S_MAX);
+    h->force_S = sub_tiles;
+    return DNATOK_OK;
 }
 
 const char *dnatok_last_error(const dnatok_t *h) { return h ? h->err.c_str() : "null handle"; }

@@ -15,3 +15,13 @@ def pytest_configure(config):
 @pytest.fixture(scope="session")
 def golden_dir():
     return os.path.join(ROOT, "tests", "golden")
+
+
+@pytest.fixture(params=[0, 1, 2, 8], ids=lambda s: f"S{s}")
+def super_tile(request):
+    """GPU parity must hold for every super-tile size of the single-pass encoder (0 = automatic)."""
+    import paper_2601_05531_b200 as dn
+    old = dn.SUPER_TILE
+    dn.SUPER_TILE = request.param
+    yield request.param
+    dn.SUPER_TILE = old

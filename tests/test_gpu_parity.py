@@ -12,7 +12,7 @@ import dnagen
 import oracle
 
 torch = pytest.importorskip("torch")
-pytestmark = pytest.mark.gpu
+pytestmark = [pytest.mark.gpu, pytest.mark.usefixtures("super_tile")]
 
 if torch.cuda.is_available():
     import paper_2601_05531_b200 as dn
