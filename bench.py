@@ -360,7 +360,7 @@ def run_ours(args) -> None:
     alg_bytes = n_bytes + (n_rec + 1) * 8 + out_bytes + pad_bytes  # bytes + offsets in, ids + CSR offsets out
     kern_ms = float(np.median(per_step_ms))
     roof = {"bound": "hbm" if tokkw["mode"] != "bpe" else "alu",
-            "kernel": "encode_tiles_v4" if tokkw["mode"] != "bpe" else "bpe_reads_kernel",
+            "kernel": "encode_tiles_v5" if tokkw["mode"] != "bpe" else "bpe_reads_kernel",
             "achieved": alg_bytes / (kern_ms * 1e-3) / 1e9, "peak": peak, "unit": "GB/s",
             "peak_source": peak_src, "algorithmic_bytes_per_launch": alg_bytes,
             "bytes_per_base": alg_bytes / max(1, bases), "kernel_ms": kern_ms,

@@ -171,8 +171,8 @@ int64_t dnatok_launch_count(const dnatok_t *h);
 /*
  * Tuning knob of the single-pass encoder: the flat byte buffer is cut into super-tiles of
  * sub_tiles x 16 KiB, the unit of the chained scan.  0 (default) = chosen per call from n_bytes and the SM
- * count; 1..8 = fixed (tests use this to exercise every size on small inputs).  Results never depend on it.
- * EINVAL outside 0..8.
+ * count; 1..4 = fixed (tests use this to exercise every size on small inputs).  Results never depend on it.
+ * EINVAL outside 0..4.
  */
 int dnatok_set_super_tile(dnatok_t *h, int32_t sub_tiles);
 

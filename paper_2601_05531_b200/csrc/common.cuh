@@ -20,7 +20,7 @@ enum : int { TAIL_PER_BASE = 0, TAIL_DROP = 1, TAIL_UNK = 2 };
 constexpr int NT = 256;                 // threads per CTA
 constexpr int LB = 64;                  // input bytes per thread
 constexpr int TB = NT * LB;             // input bytes per sub-tile (16 KiB)
-constexpr int S_MAX = 8;                // sub-tiles per super-tile (the unit of the chained scan), at most
+constexpr int S_MAX = 4;                // sub-tiles per super-tile (the unit of the chained scan), at most
 
 // ---- scan protocol -------------------------------------------------------------------
 enum : uint32_t { ST_EMPTY = 0, ST_AGG = 1, ST_INCL = 2 };

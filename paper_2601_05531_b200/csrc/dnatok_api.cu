@@ -1,7 +1,7 @@
 // dnatok_api.cu -- host side of the C-ABI declared in include/dnatok.h.
 //
 // Argument marshalling, scratch management and the pinned multi-stream scheduler; every
-// step of the hot path itself runs in the kernels of encode_v4.cuh / bpe_kernel.cuh /
+// step of the hot path itself runs in the kernels of encode_v5.cuh / bpe_kernel.cuh /
 // pad_kernel.cuh.  There is no CPU fallback anywhere in this file.
 #include "../../include/dnatok.h"
 
@@ -14,7 +14,7 @@
 
 #include "bpe_kernel.cuh"
 #include "common.cuh"
-#include "encode_v4.cuh"
+#include "encode_v5.cuh"
 #include "pad_kernel.cuh"
 
 using namespace dtk;
@@ -183,7 +183,7 @@ int launch_tiles(dnatok_t *h, EncCtx &c, const EncParams &prm, const uint8_t *d_
     int grid = (int)std::min<int64_t>(n_tiles, (int64_t)h->sm_count * h->enc_ctas_per_sm);
     tile_first_rec_kernel<<<(unsigned)((n_tiles + 1 + 255) / 256), 256, 0, st>>>(a);
     CU(cudaGetLastError());
-    encode_tiles_v4<IdT><<<grid, NT, sizeof(Smem4), st>>>(a);
+    encode_tiles_v5<IdT><<<grid, NT, sizeof(Smem5), st>>>(a);
     CU(cudaGetLastError());
     c.ticket_base += (unsigned long long)n_tiles + (unsigned long long)grid;
     h->launches += 2;
@@ -431,12 +431,12 @@ int dnatok_create(const dnatok_config *cfg_in, int device, dnatok_t **out) {
     }
     {
         // the stream of one super-tile needs more than the default 48 KiB of shared memory per CTA
-        if (cudaFuncSetAttribute(encode_tiles_v4<int32_t>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Smem4)) != cudaSuccess ||
-            cudaFuncSetAttribute(encode_tiles_v4<int16_t>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Smem4)) != cudaSuccess ||
-            cudaFuncSetAttribute(encode_tiles_v4<uint8_t>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Smem4)) != cudaSuccess)
+        if (cudaFuncSetAttribute(encode_tiles_v5<int32_t>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Smem5)) != cudaSuccess ||
+            cudaFuncSetAttribute(encode_tiles_v5<int16_t>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Smem5)) != cudaSuccess ||
+            cudaFuncSetAttribute(encode_tiles_v5<uint8_t>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Smem5)) != cudaSuccess)
             return bail(DNATOK_ECUDA);
         int nb = 0;
-        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, encode_tiles_v4<int32_t>, NT, sizeof(Smem4));
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, encode_tiles_v5<int32_t>, NT, sizeof(Smem5));
         h->enc_ctas_per_sm = std::max(nb, 1);
 
     }
