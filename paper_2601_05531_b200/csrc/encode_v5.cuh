@@ -34,6 +34,7 @@
 namespace dtk {
 
 constexpr int NW = NT / 32;
+static_assert(NW == 8, "cross-warp folds are written for 8 warps");
 constexpr int WB = 32 * LB;                  // input bytes per warp per sub-tile (2 KiB)
 constexpr int PEND = 16;                     // stream slots in front of the super-tile's kept bases (carried bases)
 constexpr int STREAM_BASES = PEND + S_MAX * TB;
@@ -64,7 +65,7 @@ struct Smem5 {
     int32_t ev_k[2][EVW];                    // kept bases before each of them (per buffer)
     uint16_t offw[NW][32];                   // per warp: exclusive kept-base prefix of each lane
     int32_t warp_cnt[2][NW];                 // by sub-tile parity
-    uint32_t warp_ls[2][NW];
+    alignas(16) uint32_t warp_ls[2][NW];
     uint32_t ls_sub[2];                      // exit line state of the sub-tile (by sub-tile parity)
     int32_t scan_tmp[NW];
     uint8_t lut[256];
@@ -335,6 +336,58 @@ __device__ __forceinline__ void emit_range(const EncArgs &A, const uint32_t *st,
                 while (i + 1 < nent && G.t[i + 1] <= j) ++i;
                 emit_token_slow<IdT>(A, st, G, i, j, gbase + (int64_t)q * R + (j - j0));
             }
+        }
+    }
+}
+
+// fast groups [qa, qb) of one segment: group q holds tokens q * R - a + (0 .. R-1); token t_lo starts at stream position u0
+template <typename IdT, int K, bool SINGLE>
+__device__ __forceinline__ void emit_fast_groups(const EncArgs &A, const uint32_t *st, int qa, int qb, int u0, int a, int t_lo,
+                                                 IdT *idsA, bool affine) {
+    constexpr int R = 16 / (int)sizeof(IdT);
+    constexpr int KS = SINGLE ? 1 : K;
+    for (int q = qa + (int)threadIdx.x; q < qb; q += NT)
+        emit_group_fast<IdT, K, SINGLE>(A, st, u0 + (q * R - a - t_lo) * KS, idsA + q * R, affine);
+}
+
+// all tokens [0, ntok) of a short segment table (at most EVW + 1 entries): per segment, the 16-byte groups that lie
+// inside its window part go through the fast path in one tight loop, the few tokens around them one per thread
+template <typename IdT>
+__device__ __forceinline__ void emit_segments(const EncArgs &A, const uint32_t *st, const SegTab &G, int nent, int ntok, int a,
+                                              int64_t gbase, int cap_rel, bool vec_ok, bool affine) {
+    constexpr int R = 16 / (int)sizeof(IdT);
+    const EncParams &P = A.prm;
+    const int kk = P.mode == MODE_KMER ? P.k : 0;        // 0: single-nt
+    IdT *idsA = reinterpret_cast<IdT *>(A.ids) + gbase;
+#pragma unroll 1
+    for (int i = 0; i < nent; ++i) {
+        const int t_lo = G.t[i], t_hi = i + 1 < nent ? G.t[i + 1] : ntok;
+        if (t_hi <= t_lo) continue;
+        const int u0 = G.src[i], w_hi = min(t_lo + G.nwin[i], t_hi);
+        int qa = 0, qb = 0;
+        if (vec_ok) {
+            qa = (t_lo + a + R - 1) / R;
+            qb = min((w_hi + a) / R, cap_rel / R);
+        }
+        if (qb > qa) {
+            switch (kk) {
+                case 0: emit_fast_groups<IdT, 1, true>(A, st, qa, qb, u0, a, t_lo, idsA, affine); break;
+                case 1: emit_fast_groups<IdT, 1, false>(A, st, qa, qb, u0, a, t_lo, idsA, false); break;
+                case 2: emit_fast_groups<IdT, 2, false>(A, st, qa, qb, u0, a, t_lo, idsA, false); break;
+                case 3: emit_fast_groups<IdT, 3, false>(A, st, qa, qb, u0, a, t_lo, idsA, false); break;
+                case 4: emit_fast_groups<IdT, 4, false>(A, st, qa, qb, u0, a, t_lo, idsA, false); break;
+                case 5: emit_fast_groups<IdT, 5, false>(A, st, qa, qb, u0, a, t_lo, idsA, false); break;
+                case 6: emit_fast_groups<IdT, 6, false>(A, st, qa, qb, u0, a, t_lo, idsA, false); break;
+                default: emit_fast_groups<IdT, 8, false>(A, st, qa, qb, u0, a, t_lo, idsA, false); break;
+            }
+            const int h1 = min(t_hi, qa * R - a), h2 = max(t_lo, qb * R - a);     // tokens before / after the fast groups
+            const int n1 = h1 - t_lo, n2 = t_hi - h2;
+            for (int x = (int)threadIdx.x; x < n1 + n2; x += NT) {
+                const int j = x < n1 ? t_lo + x : h2 + (x - n1);
+                emit_token_slow<IdT>(A, st, G, i, j, gbase + a + j);
+            }
+        } else {
+            for (int j = t_lo + (int)threadIdx.x; j < t_hi; j += NT) emit_token_slow<IdT>(A, st, G, i, j, gbase + a + j);
         }
     }
 }
@@ -695,7 +748,12 @@ __global__ void __launch_bounds__(NT, 4) encode_tiles_v5(const __grid_constant__
                         return ls;
                     };
                     uint32_t e_hr = 0, e_x = LS_LINE_START, s_hr = 0, s_x = LS_LINE_START;
-                    if (P.strip_headers) {
+                    if (P.strip_headers && !__any_sync(FULL, (nl | gt | rs | osk) != 0ull)) {
+                        // nothing in this warp's 2 KiB touches the line state: every summary is (no reset, IN_LINE)
+                        s_x = LS_IN_LINE;
+                        if (lane == 31) sm.warp_ls[sp][warp] = LS_IN_LINE;
+                        e_x = lane == 0 ? LS_LINE_START : LS_IN_LINE;
+                    } else if (P.strip_headers) {
                         bool pend0;
                         const unsigned long long ls0 = settle(ls_base | bit_at(0), pend0);
                         if (pend0) s_x = LS_LINE_START;
@@ -720,10 +778,21 @@ __global__ void __launch_bounds__(NT, 4) encode_tiles_v5(const __grid_constant__
                     unsigned long long hdr = 0;
                     if (P.strip_headers) {
                         uint32_t z_hr = 0, z_x = LS_LINE_START;          // summary of the warps before this one
+                        {
+                            const uint4 wl0 = *reinterpret_cast<const uint4 *>(&sm.warp_ls[sp][0]);
+                            const uint4 wl1 = *reinterpret_cast<const uint4 *>(&sm.warp_ls[sp][4]);
+                            const uint32_t wl[8] = {wl0.x, wl0.y, wl0.z, wl0.w, wl1.x, wl1.y, wl1.z, wl1.w};
+                            const uint32_t w_or = (wl0.x | wl0.y | wl0.z | wl0.w) | (wl1.x | wl1.y | wl1.z | wl1.w);
+                            const uint32_t w_and = (wl0.x & wl0.y & wl0.z & wl0.w) & (wl1.x & wl1.y & wl1.z & wl1.w);
+                            if (w_or == LS_IN_LINE && w_and == LS_IN_LINE) {     // all (no reset, IN_LINE)
+                                if (warp > 0) z_x = LS_IN_LINE;
+                            } else {
 #pragma unroll
-                        for (int w = 0; w < NW - 1; ++w) {
-                            const uint32_t v2 = sm.warp_ls[sp][w], g_hr = v2 >> 2, g_x = v2 & 3u;
-                            if (w < warp) { z_x = ls_apply(g_hr, g_x, z_x); z_hr |= g_hr; }
+                                for (int w = 0; w < NW - 1; ++w) {
+                                    const uint32_t g_hr = wl[w] >> 2, g_x = wl[w] & 3u;
+                                    if (w < warp) { z_x = ls_apply(g_hr, g_x, z_x); z_hr |= g_hr; }
+                                }
+                            }
                         }
                         uint32_t st_in = ls_apply(z_hr, z_x, ls_use);
                         if (tid == NT - 1) {                             // whole sub-tile: exit state, super-tile summary
@@ -755,6 +824,7 @@ __global__ void __launch_bounds__(NT, 4) encode_tiles_v5(const __grid_constant__
                         const unsigned long long mb = bb <= 0 ? 0ull : (bb >= 64 ? ~0ull : ~from_pos((int)bb));
                         keep &= ma & mb;
                     }
+                    const bool wfull = __all_sync(FULL, keep == ~0ull);  // nothing dropped in this warp's 2 KiB
                     const int n = __popcll(keep);
                     if (n == 0) { chi = clo = bad = 0ull; }
                     else if (n != 64) {
@@ -779,8 +849,11 @@ __global__ void __launch_bounds__(NT, 4) encode_tiles_v5(const __grid_constant__
                         }
                     }
                     int inc = n;
+                    if (wfull) inc = LB * (lane + 1);
+                    else {
 #pragma unroll
-                    for (int d = 1; d < 32; d <<= 1) { const int t = __shfl_up_sync(FULL, inc, d); if (lane >= d) inc += t; }
+                        for (int d = 1; d < 32; d <<= 1) { const int t = __shfl_up_sync(FULL, inc, d); if (lane >= d) inc += t; }
+                    }
                     if (lane == 31) sm.warp_cnt[sp][warp] = inc;
                     __syncthreads();                                     // ---- C: warp counts, sub-tile exit line state
 
@@ -788,7 +861,29 @@ __global__ void __launch_bounds__(NT, 4) encode_tiles_v5(const __grid_constant__
                     int woff = 0, ksub = 0;
 #pragma unroll
                     for (int w = 0; w < NW; ++w) { const int t = sm.warp_cnt[sp][w]; woff += (w < warp) ? t : 0; ksub += t; }
-                    if (n > 0) {
+                    if (wfull) {
+                        // every lane appends 64 bases: whole words, the bits shared with the lane before come by shuffle
+                        const int u = PEND + base + woff + LB * lane;
+                        const uint32_t C0 = (uint32_t)(chi >> 32), C1 = (uint32_t)chi, C2 = (uint32_t)(clo >> 32), C3 = (uint32_t)clo;
+                        const uint32_t bh = (uint32_t)(bad >> 32), bl = (uint32_t)bad;
+                        uint32_t pC3 = __shfl_up_sync(FULL, C3, 1), pbl = __shfl_up_sync(FULL, bl, 1);
+                        if (lane == 0) { pC3 = 0u; pbl = 0u; }
+                        const int cw0 = u >> 4, csh = 2 * (u & 15);      // csh, fsh are the same in every lane
+                        const uint32_t c0 = __funnelshift_r(C0, pC3, csh);
+                        if (lane == 0) { if (c0) atomicOr(&stB[cw0], c0); } else stB[cw0] = c0;
+                        stB[cw0 + 1] = __funnelshift_r(C1, C0, csh);
+                        stB[cw0 + 2] = __funnelshift_r(C2, C1, csh);
+                        stB[cw0 + 3] = __funnelshift_r(C3, C2, csh);
+                        const int fw0 = SW_CODE + (u >> 5), fsh = u & 31;
+                        const uint32_t f0 = __funnelshift_r(bh, pbl, fsh);
+                        if (lane == 0) { if (f0) atomicOr(&stB[fw0], f0); } else stB[fw0] = f0;
+                        stB[fw0 + 1] = __funnelshift_r(bl, bh, fsh);
+                        if (lane == 31) {
+                            const uint32_t c4 = __funnelshift_r(0u, C3, csh), f2 = __funnelshift_r(0u, bl, fsh);
+                            if (csh && c4) atomicOr(&stB[cw0 + 4], c4);
+                            if (fsh && f2) atomicOr(&stB[fw0 + 2], f2);
+                        }
+                    } else if (n > 0) {
                         const int u = PEND + base + woff + inc - n;      // stream position of this thread's first kept base
                         const uint32_t C0 = (uint32_t)(chi >> 32), C1 = (uint32_t)chi, C2 = (uint32_t)(clo >> 32), C3 = (uint32_t)clo;
                         const int cw0 = u >> 4, csh = 2 * (u & 15);
@@ -1005,7 +1100,7 @@ __global__ void __launch_bounds__(NT, 4) encode_tiles_v5(const __grid_constant__
             if (mA <= EVW) {
                 SegTab G; G.src = sm.seg_src[ba]; G.t = sm.seg_t[ba]; G.nwin = sm.seg_nwin[ba];
                 if (tid < mA) A.out_off[rloA + tid] = T0 + G.t[1 + tid];
-                emit_range<IdT>(A, stA, G, 0, sm.ntok, mA + 1, a, gbase, cap_rel, vec_ok, affine);
+                emit_segments<IdT>(A, stA, G, mA + 1, sm.ntok, a, gbase, cap_rel, vec_ok, affine);
             } else {
                 SegTab G; G.src = sm.ent_src; G.t = sm.ent_t; G.nwin = sm.ent_nwin;
                 if (tid == 0) { sm.ent_src[0] = sm.seg_src[ba][0]; sm.ent_t[0] = 0; sm.ent_nwin[0] = sm.seg_nwin[ba][0]; }
