@@ -64,7 +64,7 @@ struct Smem5 {
     int32_t ev_p[2][EVW];                    // super-tile positions of the first EVW record starts (by ticket parity)
     int32_t ev_k[2][EVW];                    // kept bases before each of them (per buffer)
     uint16_t offw[NW][32];                   // per warp: exclusive kept-base prefix of each lane
-    int32_t warp_cnt[2][NW];                 // by sub-tile parity
+    alignas(16) int32_t warp_cnt[2][NW];     // by sub-tile parity
     alignas(16) uint32_t warp_ls[2][NW];
     uint32_t ls_sub[2];                      // exit line state of the sub-tile (by sub-tile parity)
     int32_t scan_tmp[NW];
@@ -708,7 +708,10 @@ __global__ void __launch_bounds__(NT, 4) encode_tiles_v5(const __grid_constant__
                         }
                         chi = ((unsigned long long)C[0] << 32) | C[1];
                         clo = ((unsigned long long)C[2] << 32) | C[3];
-                        E = flags_to_plane(fb);
+                        uint32_t anyf = 0;
+#pragma unroll
+                        for (int j = 0; j < 16; ++j) anyf |= fb[j];
+                        E = anyf ? flags_to_plane(fb) : 0ull;
                         if (!P.fast_lut) E = ~0ull;
                         bad = E;
                         // runs of N: classified arithmetically too (their digit is already 2), not one LUT trip per byte
@@ -801,6 +804,9 @@ __global__ void __launch_bounds__(NT, 4) encode_tiles_v5(const __grid_constant__
                             t_x = ls_apply(z_hr, z_x, t_x); t_hr |= z_hr;
                         }
                         st_in = ls_apply(e_hr, e_x, st_in);
+                        if ((nl | gt | rs) == 0ull) {                    // no line ends or starts here: all header or none
+                            if (st_in == LS_IN_HEADER) hdr = ~0ull;
+                        } else {
                         bool pd;
                         const unsigned long long ls = settle(ls_base | (st_in == LS_LINE_START ? bit_at(0) : 0ull), pd);
                         unsigned long long hs = ls & gt;                 // header lines that start inside this thread's bytes
@@ -815,6 +821,7 @@ __global__ void __launch_bounds__(NT, 4) encode_tiles_v5(const __grid_constant__
                             const int a = first_pos(nl & from_pos(h)), bb = first_pos(rs & from_pos(h + 1));
                             const int e = (bb <= a) ? bb - 1 : a;
                             hdr |= from_pos(h) & ((e >= 63) ? ~0ull : ~from_pos(e + 1));
+                        }
                         }
                     }
                     unsigned long long keep = ~skip & ~hdr;
@@ -859,8 +866,13 @@ __global__ void __launch_bounds__(NT, 4) encode_tiles_v5(const __grid_constant__
 
                     // ================= P3: stream append; kept-base index of the record starts =========================
                     int woff = 0, ksub = 0;
+{
+                        const int4 wc0 = *reinterpret_cast<const int4 *>(&sm.warp_cnt[sp][0]);
+                        const int4 wc1 = *reinterpret_cast<const int4 *>(&sm.warp_cnt[sp][4]);
+                        const int wc[8] = {wc0.x, wc0.y, wc0.z, wc0.w, wc1.x, wc1.y, wc1.z, wc1.w};
 #pragma unroll
-                    for (int w = 0; w < NW; ++w) { const int t = sm.warp_cnt[sp][w]; woff += (w < warp) ? t : 0; ksub += t; }
+                        for (int w = 0; w < NW; ++w) { woff += (w < warp) ? wc[w] : 0; ksub += wc[w]; }
+                    }
                     if (wfull) {
                         // every lane appends 64 bases: whole words, the bits shared with the lane before come by shuffle
                         const int u = PEND + base + woff + LB * lane;
