@@ -37,7 +37,7 @@ MIB = 1 << 20
 
 
 # ----------------------------------------------------------------------------------------- workloads
-def workload_spec(config: int, scale: float = 1.0) -> dict:
+def workload_spec(config: int, scale: float = 1.0, k: int = 6) -> dict:
     """Binding-style kwargs + generator call for BASELINE.json configs[config-1]."""
     if config == 1:
         return dict(name="config1: single-nt, 16 x 65,536 bases, 60-col lines, 1% N, 5% lowercase",
@@ -48,8 +48,9 @@ def workload_spec(config: int, scale: float = 1.0) -> dict:
                     gen=("config2", dict(n_records=n)), tok=dict(mode="kmer", k=6), seq_len=0)
     if config == 3:
         tb = int((1 << 30) * scale)
-        return dict(name=f"config3: 6-mer int16, {tb} bases FASTA (80-col lines + header), log-uniform lengths",
-                    gen=("config3", dict(total_bases=tb)), tok=dict(mode="kmer", k=6, id_dtype=2), seq_len=0)
+        dt = 2 if k <= 6 else 4                       # BASELINE.json config 3: int16 for k <= 6, int32 for k = 8
+        return dict(name=f"config3: {k}-mer int{8 * dt}, {tb} bases FASTA (80-col lines + header), log-uniform lengths",
+                    gen=("config3", dict(total_bases=tb)), tok=dict(mode="kmer", k=k, id_dtype=dt), seq_len=0)
     if config == 4:
         n = max(1, int(65536 * scale))
         return dict(name=f"config4: BPE 4,092 merges, {n} reads of 500-1,500 bases, 2% N, int32",
@@ -197,7 +198,7 @@ def run_reference(args) -> None:
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    spec = workload_spec(args.config, args.scale)
+    spec = workload_spec(args.config, args.scale, args.k)
     w = generate(spec, seed=0)
     data, offs, bases = oracle_sample(w)
     cfg = oracle_config(spec, w)
@@ -265,7 +266,7 @@ def run_ours(args) -> None:
         dist.all_reduce(t, op=dist.ReduceOp.SUM)
         return float(t.item())
 
-    spec = workload_spec(args.config, args.scale)
+    spec = workload_spec(args.config, args.scale, args.k)
     tokkw = dict(spec["tok"])
     # ---- input: generated straight into pinned host memory (also the e2e source) ------------------
     t0 = time.perf_counter()
@@ -451,6 +452,7 @@ def main() -> None:
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=2)
+    ap.add_argument("--k", type=int, default=6, help="config 3 only: k of the k-mer sweep (1,2,3,4,5,6,8)")
     ap.add_argument("--scale", type=float, default=1.0, help="shrink the workload (debugging only)")
     ap.add_argument("--chunk-mib", type=int, default=64)
     ap.add_argument("--streams", type=int, default=4)
