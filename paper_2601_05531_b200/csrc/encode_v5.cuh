@@ -730,15 +730,11 @@ __global__ void __launch_bounds__(NT, 4) encode_tiles_v5(const __grid_constant__
                             const unsigned long long bq = bit_at(q);
                             rem ^= bq;
                             const uint32_t byte = (full || p0 + q < A.p_end) ? (uint32_t)__ldg(vb + q) : 0u;
-                            const uint32_t c = sm.lut[byte];
+                            // first trip: only what the line state and the keep mask need; the class of a flagged byte
+                            // is looked up in P2, and only if the byte is kept (header bytes never are)
                             if (byte == '\n') nl |= bq;
                             if (byte == '>') gt |= bq;
-                            if (c == CLS_SKIP) skip |= bq;
-                            if (c < CLS_N) bad &= ~bq;
-                            const unsigned long long cc = c < CLS_N ? c : (c == CLS_N ? 2u : 1u);
-                            const int sh = 62 - 2 * (q & 31);
-                            if (q < 32) chi = (chi & ~(3ull << sh)) | (cc << sh);
-                            else clo = (clo & ~(3ull << sh)) | (cc << sh);
+                            if (sm.lut[byte] == CLS_SKIP) skip |= bq;
                         }
                     }
                     // line state: thread summary (has_reset, exit state if the entry state is LINE_START), scanned over the warp
@@ -830,6 +826,23 @@ __global__ void __launch_bounds__(NT, 4) encode_tiles_v5(const __grid_constant__
                         const unsigned long long ma = a <= 0 ? ~0ull : from_pos((int)(a > 64 ? 64 : a));
                         const unsigned long long mb = bb <= 0 ? 0ull : (bb >= 64 ? ~0ull : ~from_pos((int)bb));
                         keep &= ma & mb;
+                    }
+                    {
+                        // second trip through the LUT: class of every kept byte the arithmetic did not prove to be ACGT
+                        const uint8_t *vb = A.bytes_al + p0;
+                        unsigned long long rem = E & keep;
+                        while (rem) {
+                            const int q = __clzll((long long)rem);
+                            const unsigned long long bq = bit_at(q);
+                            rem ^= bq;
+                            const uint32_t byte = (full || p0 + q < A.p_end) ? (uint32_t)__ldg(vb + q) : 0u;
+                            const uint32_t c = sm.lut[byte];
+                            if (c < CLS_N) bad &= ~bq;
+                            const unsigned long long cc = c < CLS_N ? c : (c == CLS_N ? 2u : 1u);
+                            const int sh = 62 - 2 * (q & 31);
+                            if (q < 32) chi = (chi & ~(3ull << sh)) | (cc << sh);
+                            else clo = (clo & ~(3ull << sh)) | (cc << sh);
+                        }
                     }
                     const bool wfull = __all_sync(FULL, keep == ~0ull);  // nothing dropped in this warp's 2 KiB
                     const int n = __popcll(keep);
@@ -990,7 +1003,7 @@ __global__ void __launch_bounds__(NT, 4) encode_tiles_v5(const __grid_constant__
         }
         __syncthreads();                                             // ---- D: stream B, record-start indices, summary
 
-        // ================= warp NW-1: next ticket; warp 0: aggregate(B), look-back(A) =============================
+        // ================= warp NW-1: next ticket; warp 1: aggregate(B); warp 0: look-back(A) ======================
         if (warp == NW - 1) {
             if (haveB) {
                 next_ticket = __shfl_sync(FULL, next_ticket, 0);
@@ -999,9 +1012,11 @@ __global__ void __launch_bounds__(NT, 4) encode_tiles_v5(const __grid_constant__
                 sm.c_tile[par ^ 1] = A.n_tiles;
             }
         }
-        if (warp == 0) {
-            const uint32_t tagA = (gen << 2) | ST_AGG, tagI = (gen << 2) | ST_INCL;
-            if (haveB) {
+        // the three one-warp jobs run side by side: warp NW-1 prepares the next super-tile, warp 1 publishes the aggregate
+        // of B, warp 0 looks back for A
+        const uint32_t tagA = (gen << 2) | ST_AGG, tagI = (gen << 2) | ST_INCL;
+        if (warp == 1 || warp == 0) {
+            if (warp == 1 && haveB) {
                 // ---- aggregate of super-tile B and the segment table of its record starts --------------------------
                 int fk, lk, closed = 0, ntok = 0;
                 if (m == 0) { fk = ktot; lk = ktot; }
@@ -1055,7 +1070,7 @@ __global__ void __launch_bounds__(NT, 4) encode_tiles_v5(const __grid_constant__
                     }
                 }
             }
-            if (haveA) {
+            if (warp == 0 && haveA) {
                 // ---- look-back for super-tile A, its inclusive prefix, its segment-table entry 0 ---------------------
                 const int ba = b ^ 1;
                 uint32_t *const stA = sm.strm[ba];
