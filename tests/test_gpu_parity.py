@@ -281,6 +281,19 @@ def test_bpe_homopolymer_runs_and_fasta_layout():
     check(data, [0, len(data)], mode="bpe", merges=merges, max_record_bytes=2048)
 
 
+def test_bpe_segment_lengths_around_the_lane_slot():
+    """segments of 383 / 384 / 385 / 1 bases: the lane-per-segment kernel holds at most 384 symbols per lane, longer
+    segments send their read to the block-per-read kernel; reads of both kinds sit side by side"""
+    rng = random.Random(7)
+    merges = dnagen.merge_table(seed=3, n_merges=200, corpus_bases=8192)
+    seg = lambda n: "".join(rng.choice("ACGT") for _ in range(n))
+    recs = [seg(383) + "N" + seg(384) + "N" + seg(1), seg(385) + "NN" + seg(2) + "N", seg(384), "N" + seg(384) + "R" + seg(50),
+            seg(1200), seg(40) + "N" + seg(700) + "N" + seg(40), "", "N", seg(1)]
+    data = np.frombuffer("".join(recs).encode(), dtype=np.uint8)
+    offs = np.cumsum([0] + [len(r) for r in recs])
+    check(data, offs, mode="bpe", merges=merges, max_record_bytes=2048)
+
+
 def test_bpe_read_longer_than_workspace_reports_capacity():
     merges = np.array([[0, 1]], dtype=np.int32)
     tok = dn.DNATok(mode="bpe", merges=merges, max_record_bytes=256)
