@@ -182,6 +182,42 @@ def test_gt_at_tile_start_and_newline_at_tile_end():
     check(data3, [0, len(data3)], mode="single_nt")
 
 
+@pytest.mark.parametrize("edge", [16384, 32768, 65536, 131072])
+def test_line_state_across_super_tile_edges(edge):
+    """The entry line state of a super-tile is read off the 128 bytes in front of it when they hold a newline or the
+    record start, else it comes from the chain (and the super-tile is redone if it was not IN_LINE).  `edge` is a
+    super-tile boundary for every super-tile size that divides it."""
+    rng = np.random.default_rng(edge)
+    acgt = lambda n: rng.choice(np.frombuffer(b"ACGT", dtype=np.uint8), size=n).tobytes()
+    cases = {
+        "newline last, '>' first": acgt(edge - 1) + b"\n" + b">hdr\n" + acgt(300) + b"\n",
+        "header starts 100 before, ends 200 after": acgt(edge - 101) + b"\n>" + b"h" * 299 + b"\n" + acgt(500),
+        "header starts 200 before (no newline in the last 128)": acgt(edge - 201) + b"\n>" + b"h" * 500 + b"\n" + acgt(500),
+        "header spans several super-tiles": acgt(50) + b"\n>" + b"h" * (edge + 70_000) + b"\n" + acgt(500),
+        "long line, no newline for 1000 bytes": acgt(edge - 1001) + b"\n" + acgt(1000 + 700) + b"\n>x\n" + acgt(9),
+        "CR LF then '>'": acgt(edge - 2) + b"\r\n" + b">hdr\r\n" + acgt(77) + b"\r\n",
+        "newline, CR at the edge, then '>'": acgt(edge - 1) + b"\n" + b"\r>hdr\n" + acgt(77),
+        "'>' mid-line at the edge": acgt(edge) + b">not a header\n" + acgt(77),
+        "record starts 60 before with '>' (record start inside the window)": None,
+    }
+    for name, data in cases.items():
+        if data is None:
+            data = acgt(edge - 60) + b">" + b"h" * 200 + b"\n" + acgt(400)
+            offs = [0, edge - 60, len(data)]
+        else:
+            offs = [0, len(data)]
+        for kw in (dict(mode="kmer", k=6), dict(mode="single_nt")):
+            check(data, offs, **kw)
+
+
+@pytest.mark.parametrize("k", [5, 6, 8])
+def test_walk_back_over_many_super_tiles(k):
+    """3 MiB in three records: with 16 KiB super-tiles the look-back walks through several windows of 32 aggregates
+    that hold no record start, carrying the open record's (q, r) and pending bases"""
+    w = dnagen.config2(n_records=3, bases=(1 << 20) + 12345, n_frac=0.002)
+    check(w.data, w.offsets, mode="kmer", k=k)
+
+
 @pytest.mark.parametrize("seed", range(12))
 def test_fuzz_fasta_like(seed):
     rng = random.Random(seed)
