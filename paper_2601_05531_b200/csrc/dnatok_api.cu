@@ -183,7 +183,11 @@ int launch_tiles(dnatok_t *h, EncCtx &c, const EncParams &prm, const uint8_t *d_
     int grid = (int)std::min<int64_t>(n_tiles, (int64_t)h->sm_count * h->enc_ctas_per_sm);
     tile_first_rec_kernel<<<(unsigned)((n_tiles + 1 + 255) / 256), 256, 0, st>>>(a);
     CU(cudaGetLastError());
-    encode_tiles_v5<IdT><<<grid, NT, sizeof(Smem5), st>>>(a);
+    // the headline shapes get a kernel with only their own emission variant compiled in (smaller instruction footprint)
+    const int kk = prm.mode == MODE_KMER ? prm.k : 0;
+    if (kk == 0) encode_tiles_v5<IdT, 0><<<grid, NT, sizeof(Smem5), st>>>(a);
+    else if (kk == 6 && sizeof(IdT) >= 2) encode_tiles_v5<IdT, 6><<<grid, NT, sizeof(Smem5), st>>>(a);
+    else encode_tiles_v5<IdT, -1><<<grid, NT, sizeof(Smem5), st>>>(a);
     CU(cudaGetLastError());
     c.ticket_base += (unsigned long long)n_tiles + (unsigned long long)grid;
     h->launches += 2;
@@ -431,12 +435,15 @@ int dnatok_create(const dnatok_config *cfg_in, int device, dnatok_t **out) {
     }
     {
         // the stream of one super-tile needs more than the default 48 KiB of shared memory per CTA
-        if (cudaFuncSetAttribute(encode_tiles_v5<int32_t>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Smem5)) != cudaSuccess ||
-            cudaFuncSetAttribute(encode_tiles_v5<int16_t>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Smem5)) != cudaSuccess ||
-            cudaFuncSetAttribute(encode_tiles_v5<uint8_t>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Smem5)) != cudaSuccess)
-            return bail(DNATOK_ECUDA);
+        const void *kernels[] = {(const void *)encode_tiles_v5<int32_t, 0>, (const void *)encode_tiles_v5<int32_t, 6>,
+                                 (const void *)encode_tiles_v5<int32_t, -1>, (const void *)encode_tiles_v5<int16_t, 0>,
+                                 (const void *)encode_tiles_v5<int16_t, 6>, (const void *)encode_tiles_v5<int16_t, -1>,
+                                 (const void *)encode_tiles_v5<uint8_t, 0>, (const void *)encode_tiles_v5<uint8_t, -1>};
+        for (const void *kf : kernels)
+            if (cudaFuncSetAttribute(kf, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Smem5)) != cudaSuccess)
+                return bail(DNATOK_ECUDA);
         int nb = 0;
-        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, encode_tiles_v5<int32_t>, NT, sizeof(Smem5));
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, encode_tiles_v5<int32_t, -1>, NT, sizeof(Smem5));
         h->enc_ctas_per_sm = std::max(nb, 1);
 
     }

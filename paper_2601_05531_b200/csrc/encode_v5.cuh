@@ -305,7 +305,7 @@ __device__ __forceinline__ int find_ent(const SegTab &G, int nent, int j) {
 }
 
 // tokens [ja, jb) (super-tile-relative) of the segment table G; `a` = T0 mod R, gbase = T0 - a
-template <typename IdT>
+template <typename IdT, int KK>
 __device__ __forceinline__ void emit_range(const EncArgs &A, const uint32_t *st, const SegTab &G, int ja, int jb, int nent, int a,
                                            int64_t gbase, int cap_rel, bool vec_ok, bool affine) {
     constexpr int R = 16 / (int)sizeof(IdT);
@@ -321,7 +321,9 @@ __device__ __forceinline__ void emit_range(const EncArgs &A, const uint32_t *st,
         if (vec_ok && hi - lo == R && jj + R <= G.nwin[i] && q * R + R <= cap_rel) {
             const int u = G.src[i] + jj * kstep;
             IdT *dst = idsA + q * R;
-            switch (kk) {
+            if constexpr (KK == 0) emit_group_fast<IdT, 1, true>(A, st, u, dst, affine);
+            else if constexpr (KK > 0) emit_group_fast<IdT, KK, false>(A, st, u, dst, false);
+            else switch (kk) {
                 case 0: emit_group_fast<IdT, 1, true>(A, st, u, dst, affine); break;
                 case 1: emit_group_fast<IdT, 1, false>(A, st, u, dst, false); break;
                 case 2: emit_group_fast<IdT, 2, false>(A, st, u, dst, false); break;
@@ -352,7 +354,7 @@ __device__ __forceinline__ void emit_fast_groups(const EncArgs &A, const uint32_
 
 // all tokens [0, ntok) of a short segment table (at most EVW + 1 entries): per segment, the 16-byte groups that lie
 // inside its window part go through the fast path in one tight loop, the few tokens around them one per thread
-template <typename IdT>
+template <typename IdT, int KK>
 __device__ __forceinline__ void emit_segments(const EncArgs &A, const uint32_t *st, const SegTab &G, int nent, int ntok, int a,
                                               int64_t gbase, int cap_rel, bool vec_ok, bool affine) {
     constexpr int R = 16 / (int)sizeof(IdT);
@@ -370,7 +372,9 @@ __device__ __forceinline__ void emit_segments(const EncArgs &A, const uint32_t *
             qb = min((w_hi + a) / R, cap_rel / R);
         }
         if (qb > qa) {
-            switch (kk) {
+            if constexpr (KK == 0) emit_fast_groups<IdT, 1, true>(A, st, qa, qb, u0, a, t_lo, idsA, affine);
+            else if constexpr (KK > 0) emit_fast_groups<IdT, KK, false>(A, st, qa, qb, u0, a, t_lo, idsA, false);
+            else switch (kk) {
                 case 0: emit_fast_groups<IdT, 1, true>(A, st, qa, qb, u0, a, t_lo, idsA, affine); break;
                 case 1: emit_fast_groups<IdT, 1, false>(A, st, qa, qb, u0, a, t_lo, idsA, false); break;
                 case 2: emit_fast_groups<IdT, 2, false>(A, st, qa, qb, u0, a, t_lo, idsA, false); break;
@@ -572,7 +576,8 @@ __device__ __forceinline__ Pre look_back(const EncArgs &A, int tile, int lane) {
 }
 
 // ======================================================================================================
-template <typename IdT>
+// KK: the emission variant compiled in -- 0 single-nt, 1..6 / 8 that k, -1 every variant behind a run-time switch
+template <typename IdT, int KK>
 __global__ void __launch_bounds__(NT, 4) encode_tiles_v5(const __grid_constant__ EncArgs A) {
     extern __shared__ __align__(16) uint8_t smem_raw[];
     Smem5 &sm = *reinterpret_cast<Smem5 *>(smem_raw);
@@ -1127,7 +1132,7 @@ __global__ void __launch_bounds__(NT, 4) encode_tiles_v5(const __grid_constant__
             if (mA <= EVW) {
                 SegTab G; G.src = sm.seg_src[ba]; G.t = sm.seg_t[ba]; G.nwin = sm.seg_nwin[ba];
                 if (tid < mA) A.out_off[rloA + tid] = T0 + G.t[1 + tid];
-                emit_segments<IdT>(A, stA, G, mA + 1, sm.ntok, a, gbase, cap_rel, vec_ok, affine);
+                emit_segments<IdT, KK>(A, stA, G, mA + 1, sm.ntok, a, gbase, cap_rel, vec_ok, affine);
             } else {
                 SegTab G; G.src = sm.ent_src; G.t = sm.ent_t; G.nwin = sm.ent_nwin;
                 if (tid == 0) { sm.ent_src[0] = sm.seg_src[ba][0]; sm.ent_t[0] = 0; sm.ent_nwin[0] = sm.seg_nwin[ba][0]; }
@@ -1150,7 +1155,7 @@ __global__ void __launch_bounds__(NT, 4) encode_tiles_v5(const __grid_constant__
                     }
                     if (c0 > 0 && tid == 0) { sm.ent_src[0] = 0; sm.ent_t[0] = tbase; sm.ent_nwin[0] = 0; }
                     __syncthreads();
-                    emit_range<IdT>(A, stA, G, c0 == 0 ? 0 : tbase, tbase + total, cm + 1, a, gbase, cap_rel, vec_ok, affine);
+                    emit_range<IdT, KK>(A, stA, G, c0 == 0 ? 0 : tbase, tbase + total, cm + 1, a, gbase, cap_rel, vec_ok, affine);
                     tbase += total;
                     __syncthreads();
                 }
