@@ -185,9 +185,18 @@ int launch_tiles(dnatok_t *h, EncCtx &c, const EncParams &prm, const uint8_t *d_
     CU(cudaGetLastError());
     // the headline shapes get a kernel with only their own emission variant compiled in (smaller instruction footprint)
     const int kk = prm.mode == MODE_KMER ? prm.k : 0;
-    if (kk == 0) encode_tiles_v5<IdT, 0><<<grid, NT, sizeof(Smem5), st>>>(a);
-    else if (kk == 6 && sizeof(IdT) >= 2) encode_tiles_v5<IdT, 6><<<grid, NT, sizeof(Smem5), st>>>(a);
-    else encode_tiles_v5<IdT, -1><<<grid, NT, sizeof(Smem5), st>>>(a);
+    const bool wide = sizeof(IdT) >= 2;                        // uint8 ids: the BPE class pass, single-nt only
+    switch (wide ? kk : 0) {
+        case 0: encode_tiles_v5<IdT, 0><<<grid, NT, sizeof(Smem5), st>>>(a); break;
+        case 1: encode_tiles_v5<IdT, wide ? 1 : 0><<<grid, NT, sizeof(Smem5), st>>>(a); break;
+        case 2: encode_tiles_v5<IdT, wide ? 2 : 0><<<grid, NT, sizeof(Smem5), st>>>(a); break;
+        case 3: encode_tiles_v5<IdT, wide ? 3 : 0><<<grid, NT, sizeof(Smem5), st>>>(a); break;
+        case 4: encode_tiles_v5<IdT, wide ? 4 : 0><<<grid, NT, sizeof(Smem5), st>>>(a); break;
+        case 5: encode_tiles_v5<IdT, wide ? 5 : 0><<<grid, NT, sizeof(Smem5), st>>>(a); break;
+        case 6: encode_tiles_v5<IdT, wide ? 6 : 0><<<grid, NT, sizeof(Smem5), st>>>(a); break;
+        case 8: encode_tiles_v5<IdT, wide ? 8 : 0><<<grid, NT, sizeof(Smem5), st>>>(a); break;
+        default: encode_tiles_v5<IdT, wide ? -1 : 0><<<grid, NT, sizeof(Smem5), st>>>(a); break;
+    }
     CU(cudaGetLastError());
     c.ticket_base += (unsigned long long)n_tiles + (unsigned long long)grid;
     h->launches += 2;
@@ -435,10 +444,11 @@ int dnatok_create(const dnatok_config *cfg_in, int device, dnatok_t **out) {
     }
     {
         // the stream of one super-tile needs more than the default 48 KiB of shared memory per CTA
-        const void *kernels[] = {(const void *)encode_tiles_v5<int32_t, 0>, (const void *)encode_tiles_v5<int32_t, 6>,
-                                 (const void *)encode_tiles_v5<int32_t, -1>, (const void *)encode_tiles_v5<int16_t, 0>,
-                                 (const void *)encode_tiles_v5<int16_t, 6>, (const void *)encode_tiles_v5<int16_t, -1>,
-                                 (const void *)encode_tiles_v5<uint8_t, 0>, (const void *)encode_tiles_v5<uint8_t, -1>};
+#define DTK_VARIANTS(T) (const void *)encode_tiles_v5<T, 0>, (const void *)encode_tiles_v5<T, 1>, (const void *)encode_tiles_v5<T, 2>, \
+                        (const void *)encode_tiles_v5<T, 3>, (const void *)encode_tiles_v5<T, 4>, (const void *)encode_tiles_v5<T, 5>, \
+                        (const void *)encode_tiles_v5<T, 6>, (const void *)encode_tiles_v5<T, 8>, (const void *)encode_tiles_v5<T, -1>
+        const void *kernels[] = {DTK_VARIANTS(int32_t), DTK_VARIANTS(int16_t), (const void *)encode_tiles_v5<uint8_t, 0>};
+#undef DTK_VARIANTS
         for (const void *kf : kernels)
             if (cudaFuncSetAttribute(kf, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Smem5)) != cudaSuccess)
                 return bail(DNATOK_ECUDA);

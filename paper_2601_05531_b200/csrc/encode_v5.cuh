@@ -160,6 +160,36 @@ __device__ __forceinline__ unsigned long long low_classes(unsigned long long t, 
     return t & ((1ull << (3 * n)) - 1ull);
 }
 
+// A lane with many flagged bytes (header text, a run of N) gets the whole warp's help: lane j looks at bytes j and
+// j + 32 of lane src's 64 bytes, the answers come back by OR-reduction.  Out of line: it runs for a few warps only
+// and the sub-tile loop is sensitive to its instruction footprint.
+struct HeavyLane { unsigned long long nl, gt, skip, n; };
+__device__ __noinline__ HeavyLane heavy_lane_flags(const EncArgs &A, const uint8_t *lut, unsigned long long E, int src,
+                                                   int64_t p0, bool full, int lane) {
+    constexpr uint32_t FULL = 0xffffffffu;
+    const uint32_t Eh = __shfl_sync(FULL, (uint32_t)(E >> 32), src), El = __shfl_sync(FULL, (uint32_t)E, src);
+    const int64_t ps = p0 + (int64_t)(src - lane) * LB;          // first byte of that lane
+    const uint32_t bit = 0x80000000u >> lane;
+    uint32_t w_nl[2] = {0, 0}, w_gt[2] = {0, 0}, w_sk[2] = {0, 0}, w_n[2] = {0, 0};
+#pragma unroll
+    for (int hh = 0; hh < 2; ++hh) {
+        if ((hh ? El : Eh) & bit) {
+            const int q = lane + 32 * hh;
+            const uint32_t byte = (full || ps + q < A.p_end) ? (uint32_t)__ldg(A.bytes_al + ps + q) : 0u;
+            if (byte == '\n') w_nl[hh] = bit;
+            if (byte == '>') w_gt[hh] = bit;
+            if (lut[byte] == CLS_SKIP) w_sk[hh] = bit;
+            if ((byte | 0x20u) == 'n') w_n[hh] = bit;
+        }
+    }
+    HeavyLane r;
+    r.nl = ((unsigned long long)__reduce_or_sync(FULL, w_nl[0]) << 32) | __reduce_or_sync(FULL, w_nl[1]);
+    r.gt = ((unsigned long long)__reduce_or_sync(FULL, w_gt[0]) << 32) | __reduce_or_sync(FULL, w_gt[1]);
+    r.skip = ((unsigned long long)__reduce_or_sync(FULL, w_sk[0]) << 32) | __reduce_or_sync(FULL, w_sk[1]);
+    r.n = ((unsigned long long)__reduce_or_sync(FULL, w_n[0]) << 32) | __reduce_or_sync(FULL, w_n[1]);
+    return r;
+}
+
 // ---- scan algebra -----------------------------------------------------------------------------------------
 // Agg: a run of consecutive super-tiles seen on its own.  Pre: everything before a point of the byte stream.
 struct Agg { uint32_t hasev; int fk, lk, closed, tn; unsigned long long tail; };
@@ -720,6 +750,7 @@ __global__ void __launch_bounds__(NT, 4) encode_tiles_v5(const __grid_constant__
                         if (!P.fast_lut) E = ~0ull;
                         bad = E;
                         // runs of N: classified arithmetically too (their digit is already 2), not one LUT trip per byte
+                        // (lanes that are still heavy afterwards -- header text -- are handled by the whole warp below)
                         if (P.fast_lut && P.fast_n && __any_sync(FULL, __popcll(E) >= 4)) {
 #pragma unroll
                             for (int j = 0; j < 16; ++j) fb[j] = is_n_word(xw[j]);
@@ -727,9 +758,24 @@ __global__ void __launch_bounds__(NT, 4) encode_tiles_v5(const __grid_constant__
                         }
                     }
                     unsigned long long skip = 0, nl = 0, gt = 0;
+                    bool coop_done = false;
+                    if (P.fast_lut) {
+                        uint32_t hv = __ballot_sync(FULL, __popcll(E) >= 4);
+                        while (hv) {
+                            const int src = __ffs(hv) - 1;
+                            hv &= hv - 1;
+                            const HeavyLane hl = heavy_lane_flags(A, sm.lut, E, src, p0, full, lane);
+                            if (lane == src) {
+                                nl = hl.nl; gt = hl.gt; skip = hl.skip;
+                                // 'N' / 'n' already carry digit 2 and stay flagged in `bad`: no second trip for them
+                                if (P.fast_n) E &= ~hl.n;
+                                coop_done = true;
+                            }
+                        }
+                    }
                     {
                         const uint8_t *vb = A.bytes_al + p0;
-                        unsigned long long rem = E;
+                        unsigned long long rem = coop_done ? 0ull : E;
                         while (rem) {
                             const int q = __clzll((long long)rem);
                             const unsigned long long bq = bit_at(q);
