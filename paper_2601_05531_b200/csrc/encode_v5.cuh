@@ -190,6 +190,41 @@ __device__ __noinline__ HeavyLane heavy_lane_flags(const EncArgs &A, const uint8
     return r;
 }
 
+// 64-bit plane (first byte at bit 63) of the bytes that are 'N' or 'n'.  Out of line: runs for few warps, and the
+// sub-tile loop is sensitive to its instruction footprint.
+__device__ __noinline__ unsigned long long n_plane(uint4 v0, uint4 v1, uint4 v2, uint4 v3) {
+    const uint32_t xw[16] = {v0.x, v0.y, v0.z, v0.w, v1.x, v1.y, v1.z, v1.w, v2.x, v2.y, v2.z, v2.w, v3.x, v3.y, v3.z, v3.w};
+    uint32_t fb[16];
+#pragma unroll
+    for (int j = 0; j < 16; ++j) fb[j] = is_n_word(xw[j]);
+    return flags_to_plane(fb);
+}
+
+// Record starts inside the 2 KiB that begin at position lo_pos, for a super-tile with many of them (events r_lo ..
+// r_lo + m of rec_offsets): sets their bits in wk[32] (one 64-bit word per lane's bytes), returns how many there are
+// and through e_lo the index of the first.  One warp, out of line (rare path).
+__device__ __noinline__ int warp_events_many(const EncArgs &A, unsigned long long *wk, int64_t r_lo, int m, int64_t lo_pos,
+                                             int lane, int &e_lo) {
+    constexpr uint32_t FULL = 0xffffffffu;
+    const int64_t hi_pos = lo_pos + WB;
+    int lo = 0, hi = m, e_cnt = 0;                               // first event at or after the warp's first byte
+    while (lo < hi) {
+        const int mid = (lo + hi) >> 1;
+        if (rec_pos(A, r_lo + mid) >= lo_pos) hi = mid; else lo = mid + 1;
+    }
+    e_lo = lo;
+    for (int e = lo; e < m; e += 32) {
+        const int ee = e + lane;
+        const int64_t pp = ee < m ? rec_pos(A, r_lo + ee) : hi_pos;
+        const uint32_t inr = __ballot_sync(FULL, pp < hi_pos);
+        if (inr && e_cnt == 0) { wk[lane] = 0ull; __syncwarp(); }
+        if (pp < hi_pos) atomicOr(&wk[(int)(pp - lo_pos) >> 6], bit_at((int)(pp - lo_pos) & 63));
+        e_cnt += __popc(inr);
+        if (inr != FULL) break;
+    }
+    return e_cnt;
+}
+
 // ---- scan algebra -----------------------------------------------------------------------------------------
 // Agg: a run of consecutive super-tiles seen on its own.  Pre: everything before a point of the byte stream.
 struct Agg { uint32_t hasev; int fk, lk, closed, tn; unsigned long long tail; };
@@ -707,22 +742,7 @@ __global__ void __launch_bounds__(NT, 4) encode_tiles_v5(const __grid_constant__
                                 rs = sm.wk[warp][lane];
                             }
                         } else {
-                            const int64_t lo_pos = t0 + wb, hi_pos = lo_pos + WB;
-                            int lo = 0, hi = m;                          // first event at or after the warp's first byte
-                            while (lo < hi) {
-                                const int mid = (lo + hi) >> 1;
-                                if (rec_pos(A, r_lo + mid) >= lo_pos) hi = mid; else lo = mid + 1;
-                            }
-                            e_lo = lo;
-                            for (int e = e_lo; e < m; e += 32) {
-                                const int ee = e + lane;
-                                const int64_t pp = ee < m ? rec_pos(A, r_lo + ee) : hi_pos;
-                                const uint32_t inr = __ballot_sync(FULL, pp < hi_pos);
-                                if (inr && e_cnt == 0) { sm.wk[warp][lane] = 0ull; __syncwarp(); }
-                                if (pp < hi_pos) atomicOr(&sm.wk[warp][(int)(pp - lo_pos) >> 6], bit_at((int)(pp - lo_pos) & 63));
-                                e_cnt += __popc(inr);
-                                if (inr != FULL) break;
-                            }
+                            e_cnt = warp_events_many(A, sm.wk[warp], r_lo, m, t0 + wb, lane, e_lo);
                             if (e_cnt) { __syncwarp(); rs = sm.wk[warp][lane]; }
                         }
                     }
@@ -752,9 +772,7 @@ __global__ void __launch_bounds__(NT, 4) encode_tiles_v5(const __grid_constant__
                         // runs of N: classified arithmetically too (their digit is already 2), not one LUT trip per byte
                         // (lanes that are still heavy afterwards -- header text -- are handled by the whole warp below)
                         if (P.fast_lut && P.fast_n && __any_sync(FULL, __popcll(E) >= 4)) {
-#pragma unroll
-                            for (int j = 0; j < 16; ++j) fb[j] = is_n_word(xw[j]);
-                            E &= ~flags_to_plane(fb);
+                            E &= ~n_plane(v[0], v[1], v[2], v[3]);
                         }
                     }
                     unsigned long long skip = 0, nl = 0, gt = 0;
