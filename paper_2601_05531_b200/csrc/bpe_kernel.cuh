@@ -16,7 +16,7 @@
 
 namespace dtk {
 
-constexpr int BPE_NT = 128;
+constexpr int BPE_NT = 256;
 constexpr uint32_t BPE_INF = 0xffffu;          // "no rule" rank / also the largest uint16
 constexpr uint32_t SYM_N = 0xffffu, SYM_UNK = 0xfffeu;   // boundary symbols (never merged, never removed)
 constexpr uint64_t HASH_EMPTY = ~0ull;
