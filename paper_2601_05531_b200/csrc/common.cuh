@@ -17,7 +17,10 @@ enum : int { MODE_SINGLE_NT = 0, MODE_KMER = 1, MODE_BPE = 2 };
 enum : int { TAIL_PER_BASE = 0, TAIL_DROP = 1, TAIL_UNK = 2 };
 
 // ---- tile geometry -------------------------------------------------------------------
-constexpr int NT = 256;                 // threads per CTA
+#ifndef DTK_NT
+#define DTK_NT 256
+#endif
+constexpr int NT = DTK_NT;              // threads per CTA of the encode kernel
 constexpr int LB = 64;                  // input bytes per thread
 constexpr int TB = NT * LB;             // input bytes per sub-tile (16 KiB)
 constexpr int S_MAX = 4;                // sub-tiles per super-tile (the unit of the chained scan), at most

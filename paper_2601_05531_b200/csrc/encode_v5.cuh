@@ -34,7 +34,7 @@
 namespace dtk {
 
 constexpr int NW = NT / 32;
-static_assert(NW == 8, "cross-warp folds are written for 8 warps");
+static_assert(NW % 4 == 0, "warp summaries are read four at a time");
 constexpr int WB = 32 * LB;                  // input bytes per warp per sub-tile (2 KiB)
 constexpr int PEND = 16;                     // stream slots in front of the super-tile's kept bases (carried bases)
 constexpr int STREAM_BASES = PEND + S_MAX * TB;
@@ -79,7 +79,7 @@ struct Smem5 {
     int32_t tok0, ntok;                      // emission: tokens of the open record's piece, tokens of the super-tile
     long long T0;                            // global index of the super-tile's first token
 };
-static_assert(sizeof(Smem5) <= 56 * 1024, "four CTAs per SM");
+static_assert(sizeof(Smem5) <= 56 * 1024 * (NT / 256), "1024 threads per SM");
 
 // ---------------------------------------------------------------------------------------- small helpers
 __device__ __forceinline__ unsigned long long bit_at(int q) { return 0x8000000000000000ull >> q; }          // q in 0..63
@@ -643,7 +643,7 @@ __device__ __forceinline__ Pre look_back(const EncArgs &A, int tile, int lane) {
 // ======================================================================================================
 // KK: the emission variant compiled in -- 0 single-nt, 1..6 / 8 that k, -1 every variant behind a run-time switch
 template <typename IdT, int KK>
-__global__ void __launch_bounds__(NT, 4) encode_tiles_v5(const __grid_constant__ EncArgs A) {
+__global__ void __launch_bounds__(NT, 1024 / NT) encode_tiles_v5(const __grid_constant__ EncArgs A) {
     extern __shared__ __align__(16) uint8_t smem_raw[];
     Smem5 &sm = *reinterpret_cast<Smem5 *>(smem_raw);
     constexpr uint32_t FULL = 0xffffffffu;
@@ -659,7 +659,7 @@ __global__ void __launch_bounds__(NT, 4) encode_tiles_v5(const __grid_constant__
     const bool vec_ok = (reinterpret_cast<uintptr_t>(A.ids) & 15) == 0 &&
                         (P.mode != MODE_KMER || (k >= 1 && k <= 6) || k == 8);
 
-    sm.lut[tid] = A.lut[tid];
+    if (tid < 256) sm.lut[tid] = A.lut[tid];
     __syncthreads();
     unsigned long long next_ticket = 0;
     if (warp == NW - 1) {
@@ -847,11 +847,13 @@ __global__ void __launch_bounds__(NT, 4) encode_tiles_v5(const __grid_constant__
                     if (P.strip_headers) {
                         uint32_t z_hr = 0, z_x = LS_LINE_START;          // summary of the warps before this one
                         {
-                            const uint4 wl0 = *reinterpret_cast<const uint4 *>(&sm.warp_ls[sp][0]);
-                            const uint4 wl1 = *reinterpret_cast<const uint4 *>(&sm.warp_ls[sp][4]);
-                            const uint32_t wl[8] = {wl0.x, wl0.y, wl0.z, wl0.w, wl1.x, wl1.y, wl1.z, wl1.w};
-                            const uint32_t w_or = (wl0.x | wl0.y | wl0.z | wl0.w) | (wl1.x | wl1.y | wl1.z | wl1.w);
-                            const uint32_t w_and = (wl0.x & wl0.y & wl0.z & wl0.w) & (wl1.x & wl1.y & wl1.z & wl1.w);
+                            uint32_t wl[NW], w_or = 0u, w_and = ~0u;
+#pragma unroll
+                            for (int q4 = 0; q4 < NW / 4; ++q4) {
+                                const uint4 t4 = *reinterpret_cast<const uint4 *>(&sm.warp_ls[sp][4 * q4]);
+                                wl[4 * q4] = t4.x; wl[4 * q4 + 1] = t4.y; wl[4 * q4 + 2] = t4.z; wl[4 * q4 + 3] = t4.w;
+                                w_or |= (t4.x | t4.y) | (t4.z | t4.w); w_and &= (t4.x & t4.y) & (t4.z & t4.w);
+                            }
                             if (w_or == LS_IN_LINE && w_and == LS_IN_LINE) {     // all (no reset, IN_LINE)
                                 if (warp > 0) z_x = LS_IN_LINE;
                             } else {
@@ -949,9 +951,12 @@ __global__ void __launch_bounds__(NT, 4) encode_tiles_v5(const __grid_constant__
                     // ================= P3: stream append; kept-base index of the record starts =========================
                     int woff = 0, ksub = 0;
 {
-                        const int4 wc0 = *reinterpret_cast<const int4 *>(&sm.warp_cnt[sp][0]);
-                        const int4 wc1 = *reinterpret_cast<const int4 *>(&sm.warp_cnt[sp][4]);
-                        const int wc[8] = {wc0.x, wc0.y, wc0.z, wc0.w, wc1.x, wc1.y, wc1.z, wc1.w};
+                        int wc[NW];
+#pragma unroll
+                        for (int q4 = 0; q4 < NW / 4; ++q4) {
+                            const int4 t4 = *reinterpret_cast<const int4 *>(&sm.warp_cnt[sp][4 * q4]);
+                            wc[4 * q4] = t4.x; wc[4 * q4 + 1] = t4.y; wc[4 * q4 + 2] = t4.z; wc[4 * q4 + 3] = t4.w;
+                        }
 #pragma unroll
                         for (int w = 0; w < NW; ++w) { woff += (w < warp) ? wc[w] : 0; ksub += wc[w]; }
                     }
