@@ -79,7 +79,7 @@ struct Smem5 {
     int32_t tok0, ntok;                      // emission: tokens of the open record's piece, tokens of the super-tile
     long long T0;                            // global index of the super-tile's first token
 };
-static_assert(sizeof(Smem5) <= 56 * 1024 * (NT / 256), "1024 threads per SM");
+static_assert(sizeof(Smem5) <= (NT >= 256 ? 56 * 1024 * (NT / 256) : 32 * 1024), "shared memory per CTA");
 
 // ---------------------------------------------------------------------------------------- small helpers
 __device__ __forceinline__ unsigned long long bit_at(int q) { return 0x8000000000000000ull >> q; }          // q in 0..63
