@@ -918,7 +918,22 @@ __global__ void __launch_bounds__(NT, 1024 / NT) encode_tiles_v5(const __grid_co
                     const bool wfull = __all_sync(FULL, keep == ~0ull);  // nothing dropped in this warp's 2 KiB
                     const int n = __popcll(keep);
                     if (n == 0) { chi = clo = bad = 0ull; }
-                    else if (n != 64) {
+                    else if (n == 63) {
+                        // one dropped byte (the newline of a wrapped FASTA line): its flag bit and its two code bits go
+                        const int lo = __ffsll((long long)~keep) - 1;                      // plane bit of the dropped byte
+                        const unsigned long long lm = (1ull << lo) - 1ull;
+                        bad = (bad & ~(lm | (1ull << lo))) | ((bad & lm) << 1);
+                        if (lo >= 32) {
+                            const int pb = 2 * lo - 64;                                    // its code bits: chi bits pb, pb + 1
+                            const unsigned long long up = pb + 2 < 64 ? (~0ull << (pb + 2)) : 0ull;
+                            chi = (chi & up) | ((chi & ((1ull << pb) - 1ull)) << 2) | (clo >> 62);
+                            clo <<= 2;
+                        } else {
+                            const int pb = 2 * lo;                                         // clo bits pb, pb + 1
+                            const unsigned long long up = pb + 2 < 64 ? (~0ull << (pb + 2)) : 0ull;
+                            clo = (clo & up) | ((clo & ((1ull << pb) - 1ull)) << 2);
+                        }
+                    } else if (n != 64) {
                         // delete the dropped runs from the planes, last run first so earlier positions stay valid
                         unsigned long long drop = ~keep;
                         while (drop) {
