@@ -822,11 +822,16 @@ __global__ void __launch_bounds__(NT, 1024 / NT) encode_tiles_v5(const __grid_co
                         if (lane == 31) sm.warp_ls[sp][warp] = LS_IN_LINE;
                         e_x = lane == 0 ? LS_LINE_START : LS_IN_LINE;
                     } else if (P.strip_headers) {
-                        bool pend0;
-                        const unsigned long long ls0 = settle(ls_base | bit_at(0), pend0);
-                        if (pend0) s_x = LS_LINE_START;
-                        else if (!ls0) s_x = LS_LINE_START;
-                        else s_x = (gt & (ls0 & (~ls0 + 1ull))) ? LS_IN_HEADER : LS_IN_LINE;   // lowest set bit = last line start
+                        if ((gt | osk) == 0ull) {
+                            // no '>' and nothing to settle over: after the last byte the line is open unless that byte is '\n'
+                            s_x = (nl & 1ull) ? LS_LINE_START : LS_IN_LINE;
+                        } else {
+                            bool pend0;
+                            const unsigned long long ls0 = settle(ls_base | bit_at(0), pend0);
+                            if (pend0) s_x = LS_LINE_START;
+                            else if (!ls0) s_x = LS_LINE_START;
+                            else s_x = (gt & (ls0 & (~ls0 + 1ull))) ? LS_IN_HEADER : LS_IN_LINE;   // lowest set bit = last line start
+                        }
                         s_hr = (nl | rs) != 0;
 #pragma unroll
                         for (int d = 1; d < 32; d <<= 1) {
@@ -873,6 +878,8 @@ __global__ void __launch_bounds__(NT, 1024 / NT) encode_tiles_v5(const __grid_co
                         st_in = ls_apply(e_hr, e_x, st_in);
                         if ((nl | gt | rs) == 0ull) {                    // no line ends or starts here: all header or none
                             if (st_in == LS_IN_HEADER) hdr = ~0ull;
+                        } else if (gt == 0ull && st_in != LS_IN_HEADER) {
+                            // no '>' here and not inside a header: nothing of this thread's bytes is header
                         } else {
                         bool pd;
                         const unsigned long long ls = settle(ls_base | (st_in == LS_LINE_START ? bit_at(0) : 0ull), pd);
