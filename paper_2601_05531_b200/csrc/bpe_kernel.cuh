@@ -50,33 +50,51 @@ __device__ __forceinline__ uint32_t bpe_rank(const BpeArgs &A, uint32_t l, uint3
     }
 }
 
-// block-wide exclusive scan (BPE_NT threads)
-__device__ __forceinline__ int bpe_exscan(int v, int *warp_tmp, int &total) {
+// block-wide exclusive scan (BPE_NT threads), one barrier: consecutive calls alternate between the two halves of
+// warp_tmp (pp), so a warp still reading one half never meets the writes of the next call
+__device__ __forceinline__ int bpe_exscan(int v, int (*warp_tmp)[BPE_NT / 32], int &pp, int &total) {
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     int inc = v;
 #pragma unroll
     for (int d = 1; d < 32; d <<= 1) { int t = __shfl_up_sync(0xffffffffu, inc, d); if (lane >= d) inc += t; }
-    if (lane == 31) warp_tmp[warp] = inc;
+    if (lane == 31) warp_tmp[pp][warp] = inc;
     __syncthreads();
     int woff = 0, tot = 0;
 #pragma unroll
-    for (int w = 0; w < BPE_NT / 32; ++w) { int t = warp_tmp[w]; if (w < warp) woff += t; tot += t; }
-    __syncthreads();
+    for (int w = 0; w < BPE_NT / 32; ++w) { int t = warp_tmp[pp][w]; if (w < warp) woff += t; tot += t; }
+    pp ^= 1;
     total = tot;
     return woff + inc - v;
 }
 
-// dynamic shared memory layout: sym[2][cap] rnk[2][cap] seg[2][cap] src[cap] segmin[cap+1], all uint16
+// minimum of rank rk into the 16-bit slot of segment sg (two slots per 32-bit word, CAS on the word)
+__device__ __forceinline__ void bpe_seg_min(uint16_t *segmin, uint32_t sg, uint32_t rk) {
+    uint32_t *w = reinterpret_cast<uint32_t *>(segmin) + (sg >> 1);
+    uint32_t old = *w;
+    for (;;) {
+        const uint32_t half = (sg & 1) ? (old >> 16) : (old & 0xffffu);
+        if (half <= rk) break;
+        const uint32_t neu = (sg & 1) ? ((old & 0xffffu) | (rk << 16)) : ((old & 0xffff0000u) | rk);
+        const uint32_t got = atomicCAS(w, old, neu);
+        if (got == old) break;
+        old = got;
+    }
+}
+
+// dynamic shared memory layout: sym[2][cap] rnk[2][cap] seg[2][cap] src[cap] segmin[2][cap+2], all uint16.
+// One round = compaction pass (one barrier per chunk of BPE_NT symbols) -> barrier -> rank pass, which also collects
+// the next round's per-segment minima into the other segmin buffer -> barrier.
 __global__ void __launch_bounds__(BPE_NT) bpe_reads_kernel(const __grid_constant__ BpeArgs A) {
     extern __shared__ __align__(16) uint16_t sh[];
-    __shared__ int warp_tmp[BPE_NT / 32];
-    __shared__ int s_any;
+    __shared__ int warp_tmp[2][BPE_NT / 32];
+    __shared__ int s_any[2];
     const int cap = A.cap, tid = threadIdx.x;
     uint16_t *symb[2] = {sh, sh + cap};
     uint16_t *rnkb[2] = {sh + 2 * cap, sh + 3 * cap};
     uint16_t *segb[2] = {sh + 4 * cap, sh + 5 * cap};
     uint16_t *src = sh + 6 * cap;
-    uint16_t *segmin = sh + 7 * cap;
+    uint16_t *sminb[2] = {sh + 7 * cap, sh + 8 * cap + 2};
+    int pp = 0;
 
     for (int64_t r = blockIdx.x; r < A.n_rec; r += gridDim.x) {
         const int64_t k0 = A.koff[r];
@@ -86,65 +104,47 @@ __global__ void __launch_bounds__(BPE_NT) bpe_reads_kernel(const __grid_constant
             if (tid == 0) { A.status[0] = 1u; A.tok_cnt[r] = 0; }
             continue;
         }
-        int n = (int)n64, cur = 0;
+        int n = (int)n64, cur = 0, ms = 0;
         // ---- load symbols, segment ids (a boundary symbol forms its own segment) --------
         // seg id = number of "segment starts" at or before i, minus 1; a start is i == 0, a boundary,
         // or the position right after a boundary.
-        for (int base = 0; base < n; base += BPE_NT) {       // chunked so the scan carries across chunks
-            int i = base + tid;
-            uint32_t c = (i < n) ? A.cls[k0 + i] : 0u;
-            uint32_t s = c < CLS_N ? c : (c == CLS_N ? SYM_N : SYM_UNK);
-            if (i < n) symb[0][i] = (uint16_t)s;
+        for (int i = tid; i < n; i += BPE_NT) {
+            const uint32_t c = A.cls[k0 + i];
+            symb[0][i] = (uint16_t)(c < CLS_N ? c : (c == CLS_N ? SYM_N : SYM_UNK));
         }
+        for (int i = tid; i <= n; i += BPE_NT) sminb[0][i] = (uint16_t)BPE_INF;     // at most n segments
+        if (tid == 0) { s_any[0] = 0; }
         __syncthreads();
         int seg_base = 0;
-        for (int base = 0; base < n; base += BPE_NT) {
+        for (int base = 0; base < n; base += BPE_NT) {       // chunked so the scan carries across chunks
             int i = base + tid;
             int start = 0;
             if (i < n) {
-                bool b = symb[0][i] >= SYM_UNK;
+                bool bd = symb[0][i] >= SYM_UNK;
                 bool pb = (i > 0) && symb[0][i - 1] >= SYM_UNK;
-                start = (i == 0 || b || pb) ? 1 : 0;
+                start = (i == 0 || bd || pb) ? 1 : 0;
             }
             int tot;
-            int ex = bpe_exscan(start, warp_tmp, tot);
-            if (i < n) segb[0][i] = (uint16_t)(seg_base + ex + start - 1);
+            int ex = bpe_exscan(start, warp_tmp, pp, tot);
+            if (i < n) {
+                const uint32_t sg = (uint32_t)(seg_base + ex + start - 1);
+                segb[0][i] = (uint16_t)sg;
+                const uint32_t rk = (i + 1 < n) ? bpe_rank(A, symb[0][i], symb[0][i + 1]) : BPE_INF;
+                rnkb[0][i] = (uint16_t)rk;
+                if (rk != BPE_INF) { bpe_seg_min(sminb[0], sg, rk); s_any[0] = 1; }
+            }
             seg_base += tot;
         }
-        for (int i = tid; i < n; i += BPE_NT)
-            rnkb[0][i] = (uint16_t)((i + 1 < n) ? bpe_rank(A, symb[0][i], symb[0][i + 1]) : BPE_INF);
         __syncthreads();
 
         // ---- rounds ----------------------------------------------------------------------
         for (;;) {
-            uint16_t *sym = symb[cur], *rnk = rnkb[cur], *seg = segb[cur];
-            uint16_t *sym2 = symb[cur ^ 1], *rnk2 = rnkb[cur ^ 1], *seg2 = segb[cur ^ 1];
-            if (tid == 0) s_any = 0;
-            for (int i = tid; i <= seg_base; i += BPE_NT) segmin[i] = (uint16_t)BPE_INF;
-            __syncthreads();
-            // per-segment minimum rank (16-bit values packed two per word: CAS-free atomicMin on the half)
-            bool any = false;
-            for (int i = tid; i < n; i += BPE_NT) {
-                uint32_t rk = rnk[i];
-                if (rk != BPE_INF) {
-                    any = true;
-                    uint32_t sg = seg[i];
-                    uint32_t *w = reinterpret_cast<uint32_t *>(segmin) + (sg >> 1);
-                    // min on one 16-bit half: try until our value is not smaller any more
-                    uint32_t old = *w;
-                    for (;;) {
-                        uint32_t half = (sg & 1) ? (old >> 16) : (old & 0xffffu);
-                        if (half <= rk) break;
-                        uint32_t neu = (sg & 1) ? ((old & 0xffffu) | (rk << 16)) : ((old & 0xffff0000u) | rk);
-                        uint32_t got = atomicCAS(w, old, neu);
-                        if (got == old) break;
-                        old = got;
-                    }
-                }
-            }
-            if (any) s_any = 1;
-            __syncthreads();
-            if (!s_any) break;
+            if (!s_any[ms]) break;
+            uint16_t *sym = symb[cur], *rnk = rnkb[cur], *seg = segb[cur], *segmin = sminb[ms];
+            uint16_t *sym2 = symb[cur ^ 1], *rnk2 = rnkb[cur ^ 1], *seg2 = segb[cur ^ 1], *smin2 = sminb[ms ^ 1];
+            // the other minima buffer gets ready for the rank pass of this round
+            for (int i = tid; i <= seg_base; i += BPE_NT) smin2[i] = (uint16_t)BPE_INF;
+            if (tid == 0) s_any[ms ^ 1] = 0;
             // flags, run parity, compaction
             int carry = 0;
             for (int base = 0; base < n; base += BPE_NT) {
@@ -165,7 +165,7 @@ __global__ void __launch_bounds__(BPE_NT) bpe_reads_kernel(const __grid_constant
                     keep = !(i > 0 && merges(i - 1));
                 }
                 int tot;
-                int w = carry + bpe_exscan(keep ? 1 : 0, warp_tmp, tot);
+                int w = carry + bpe_exscan(keep ? 1 : 0, warp_tmp, pp, tot);
                 if (keep) {
                     sym2[w] = merge ? (uint16_t)(4u + rnk[i]) : sym[i];
                     seg2[w] = seg[i];
@@ -175,6 +175,7 @@ __global__ void __launch_bounds__(BPE_NT) bpe_reads_kernel(const __grid_constant
             }
             __syncthreads();
             const int n2 = carry;
+            bool any = false;
             for (int w = tid; w < n2; w += BPE_NT) {
                 uint32_t rk = BPE_INF;
                 if (w + 1 < n2) {
@@ -182,8 +183,10 @@ __global__ void __launch_bounds__(BPE_NT) bpe_reads_kernel(const __grid_constant
                     else rk = rnk[src[w]];
                 }
                 rnk2[w] = (uint16_t)rk;
+                if (rk != BPE_INF) { any = true; bpe_seg_min(smin2, seg2[w], rk); }
             }
-            n = n2; cur ^= 1;
+            if (any) s_any[ms ^ 1] = 1;
+            n = n2; cur ^= 1; ms ^= 1;
             __syncthreads();
         }
         // ---- write token numbers --------------------------------------------------------
