@@ -81,6 +81,24 @@ __device__ __forceinline__ void bpe_seg_min(uint16_t *segmin, uint32_t sg, uint3
     }
 }
 
+// ranks of one warp's 32 consecutive symbols into the per-segment minima: segments are contiguous, so a segmented
+// min-scan over the warp leaves each run's minimum in its last lane, which alone touches shared memory
+__device__ __forceinline__ bool bpe_warp_seg_min(uint16_t *segmin, uint32_t sg, uint32_t rk, bool valid) {
+    constexpr uint32_t FULL = 0xffffffffu;
+    const int lane = threadIdx.x & 31;
+    if (!valid) { sg = 0xffffffffu; rk = BPE_INF; }
+    uint32_t v = rk;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+        const uint32_t t = __shfl_up_sync(FULL, v, d), st = __shfl_up_sync(FULL, sg, d);
+        if (lane >= d && st == sg) v = min(v, t);
+    }
+    const uint32_t nsg = __shfl_down_sync(FULL, sg, 1);
+    const bool last = lane == 31 || nsg != sg;
+    if (valid && last && v != BPE_INF) bpe_seg_min(segmin, sg, v);
+    return __any_sync(FULL, valid && rk != BPE_INF);
+}
+
 // dynamic shared memory layout: sym[2][cap] rnk[2][cap] seg[2][cap] src[cap] segmin[2][cap+2], all uint16.
 // One round = compaction pass (one barrier per chunk of BPE_NT symbols) -> barrier -> rank pass, which also collects
 // the next round's per-segment minima into the other segmin buffer -> barrier.
@@ -126,13 +144,14 @@ __global__ void __launch_bounds__(BPE_NT) bpe_reads_kernel(const __grid_constant
             }
             int tot;
             int ex = bpe_exscan(start, warp_tmp, pp, tot);
+            uint32_t sg = 0, rk = BPE_INF;
             if (i < n) {
-                const uint32_t sg = (uint32_t)(seg_base + ex + start - 1);
+                sg = (uint32_t)(seg_base + ex + start - 1);
                 segb[0][i] = (uint16_t)sg;
-                const uint32_t rk = (i + 1 < n) ? bpe_rank(A, symb[0][i], symb[0][i + 1]) : BPE_INF;
+                rk = (i + 1 < n) ? bpe_rank(A, symb[0][i], symb[0][i + 1]) : BPE_INF;
                 rnkb[0][i] = (uint16_t)rk;
-                if (rk != BPE_INF) { bpe_seg_min(sminb[0], sg, rk); s_any[0] = 1; }
             }
+            if (bpe_warp_seg_min(sminb[0], sg, rk, i < n) && (tid & 31) == 0) s_any[0] = 1;
             seg_base += tot;
         }
         __syncthreads();
@@ -150,7 +169,7 @@ __global__ void __launch_bounds__(BPE_NT) bpe_reads_kernel(const __grid_constant
             for (int base = 0; base < n; base += BPE_NT) {
                 int i = base + tid;
                 bool keep = false, merge = false;
-                if (i < n) {
+                {
                     auto fires = [&](int j) -> bool {            // pair (j, j+1) is selected (before overlap rule)
                         uint32_t rk = rnk[j];
                         return rk != BPE_INF && rk == segmin[seg[j]];
@@ -161,8 +180,17 @@ __global__ void __launch_bounds__(BPE_NT) bpe_reads_kernel(const __grid_constant
                         while (j - 1 - c >= 0 && fires(j - 1 - c)) ++c;
                         return (c & 1) == 0;
                     };
-                    merge = merges(i);
-                    keep = !(i > 0 && merges(i - 1));
+                    // one look at the symbol's own pair; the run of selected pairs in front of it comes from the warp's
+                    // ballot, and only a run that reaches the warp's first lane is followed back through shared memory
+                    const int ln = tid & 31;
+                    const bool f = i < n && fires(i);
+                    const uint32_t Fw = __ballot_sync(0xffffffffu, f);
+                    int c = ln ? __clz(~(Fw << (32 - ln))) : 0;  // selected pairs directly in front, inside the warp
+                    if (c > ln) c = ln;
+                    if (f && c == ln) { int j = i - ln - 1; while (j >= 0 && fires(j)) { ++c; --j; } }
+                    merge = f && (c & 1) == 0;
+                    const bool pm = __shfl_up_sync(0xffffffffu, merge, 1);
+                    if (i < n) keep = !(ln ? pm : (i > 0 && merges(i - 1)));
                 }
                 int tot;
                 int w = carry + bpe_exscan(keep ? 1 : 0, warp_tmp, pp, tot);
@@ -176,16 +204,20 @@ __global__ void __launch_bounds__(BPE_NT) bpe_reads_kernel(const __grid_constant
             __syncthreads();
             const int n2 = carry;
             bool any = false;
-            for (int w = tid; w < n2; w += BPE_NT) {
-                uint32_t rk = BPE_INF;
-                if (w + 1 < n2) {
-                    if (src[w] == 0xffffu || src[w + 1] == 0xffffu) rk = bpe_rank(A, sym2[w], sym2[w + 1]);
-                    else rk = rnk[src[w]];
+            for (int base = 0; base < n2; base += BPE_NT) {
+                const int w = base + tid;
+                uint32_t rk = BPE_INF, sg = 0;
+                if (w < n2) {
+                    if (w + 1 < n2) {
+                        if (src[w] == 0xffffu || src[w + 1] == 0xffffu) rk = bpe_rank(A, sym2[w], sym2[w + 1]);
+                        else rk = rnk[src[w]];
+                    }
+                    rnk2[w] = (uint16_t)rk;
+                    sg = seg2[w];
                 }
-                rnk2[w] = (uint16_t)rk;
-                if (rk != BPE_INF) { any = true; bpe_seg_min(smin2, seg2[w], rk); }
+                any |= bpe_warp_seg_min(smin2, sg, rk, w < n2);
             }
-            if (any) s_any[ms ^ 1] = 1;
+            if (any && (tid & 31) == 0) s_any[ms ^ 1] = 1;
             n = n2; cur ^= 1; ms ^= 1;
             __syncthreads();
         }
