@@ -50,21 +50,26 @@ __device__ __forceinline__ uint32_t bpe_rank(const BpeArgs &A, uint32_t l, uint3
     }
 }
 
-// block-wide exclusive scan (BPE_NT threads), one barrier: consecutive calls alternate between the two halves of
-// warp_tmp (pp), so a warp still reading one half never meets the writes of the next call
-__device__ __forceinline__ int bpe_exscan(int v, int (*warp_tmp)[BPE_NT / 32], int &pp, int &total) {
+// block-wide exclusive count of a flag (BPE_NT threads), one barrier: ballot + popc inside the warp, the warp totals
+// through shared memory.  Consecutive calls alternate between the two halves of warp_tmp (pp), so a warp still
+// reading one half never meets the writes of the next call.
+__device__ __forceinline__ int bpe_exscan(bool f, int (*warp_tmp)[BPE_NT / 32], int &pp, int &total) {
+    static_assert((BPE_NT / 32) % 4 == 0, "warp totals are read four at a time");
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    int inc = v;
-#pragma unroll
-    for (int d = 1; d < 32; d <<= 1) { int t = __shfl_up_sync(0xffffffffu, inc, d); if (lane >= d) inc += t; }
-    if (lane == 31) warp_tmp[pp][warp] = inc;
+    const uint32_t b = __ballot_sync(0xffffffffu, f);
+    if (lane == 0) warp_tmp[pp][warp] = __popc(b);
     __syncthreads();
     int woff = 0, tot = 0;
 #pragma unroll
-    for (int w = 0; w < BPE_NT / 32; ++w) { int t = warp_tmp[pp][w]; if (w < warp) woff += t; tot += t; }
+    for (int q = 0; q < BPE_NT / 128; ++q) {
+        const int4 t = *reinterpret_cast<const int4 *>(&warp_tmp[pp][4 * q]);
+        const int v[4] = {t.x, t.y, t.z, t.w};
+#pragma unroll
+        for (int j = 0; j < 4; ++j) { if (4 * q + j < warp) woff += v[j]; tot += v[j]; }
+    }
     pp ^= 1;
     total = tot;
-    return woff + inc - v;
+    return woff + __popc(b & ((1u << lane) - 1u));
 }
 
 // minimum of rank rk into the 16-bit slot of segment sg (two slots per 32-bit word, CAS on the word)
@@ -104,7 +109,7 @@ __device__ __forceinline__ bool bpe_warp_seg_min(uint16_t *segmin, uint32_t sg, 
 // the next round's per-segment minima into the other segmin buffer -> barrier.
 __global__ void __launch_bounds__(BPE_NT) bpe_reads_kernel(const __grid_constant__ BpeArgs A) {
     extern __shared__ __align__(16) uint16_t sh[];
-    __shared__ int warp_tmp[2][BPE_NT / 32];
+    __shared__ __align__(16) int warp_tmp[2][BPE_NT / 32];
     __shared__ int s_any[2];
     const int cap = A.cap, tid = threadIdx.x;
     uint16_t *symb[2] = {sh, sh + cap};
@@ -143,7 +148,7 @@ __global__ void __launch_bounds__(BPE_NT) bpe_reads_kernel(const __grid_constant
                 start = (i == 0 || bd || pb) ? 1 : 0;
             }
             int tot;
-            int ex = bpe_exscan(start, warp_tmp, pp, tot);
+            int ex = bpe_exscan(start != 0, warp_tmp, pp, tot);
             uint32_t sg = 0, rk = BPE_INF;
             if (i < n) {
                 sg = (uint32_t)(seg_base + ex + start - 1);
@@ -193,7 +198,7 @@ __global__ void __launch_bounds__(BPE_NT) bpe_reads_kernel(const __grid_constant
                     if (i < n) keep = !(ln ? pm : (i > 0 && merges(i - 1)));
                 }
                 int tot;
-                int w = carry + bpe_exscan(keep ? 1 : 0, warp_tmp, pp, tot);
+                int w = carry + bpe_exscan(keep, warp_tmp, pp, tot);
                 if (keep) {
                     sym2[w] = merge ? (uint16_t)(4u + rnk[i]) : sym[i];
                     seg2[w] = seg[i];
