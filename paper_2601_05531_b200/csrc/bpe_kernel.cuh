@@ -20,6 +20,7 @@ constexpr int BPE_NT = 256;
 constexpr uint32_t BPE_INF = 0xffffu;          // "no rule" rank / also the largest uint16
 constexpr uint32_t SYM_N = 0xffffu, SYM_UNK = 0xfffeu;   // boundary symbols (never merged, never removed)
 constexpr uint64_t HASH_EMPTY = ~0ull;
+constexpr uint32_t SYM_HOLE = 0xfffdu;          // tmp_tok entry that holds no token (the gather kernel drops it)
 
 struct BpeArgs {
     const uint8_t *cls;            // compact kept classes of all reads (pass A output)
@@ -28,7 +29,7 @@ struct BpeArgs {
     const uint64_t *table;         // open-addressing hash: (left<<16|right)<<32 | rank
     uint32_t table_mask;
     int32_t cap;                   // symbols per read the shared-memory workspace can hold
-    uint16_t *tmp_tok;             // token numbers of read r at tmp_tok[koff[r] ...)
+    uint16_t *tmp_tok;             // per kept base of read r: a token of the segment that started there, or SYM_HOLE
     int32_t *tok_cnt;              // [n_rec] tokens per read
     uint32_t *status;
 };
@@ -104,19 +105,24 @@ __device__ __forceinline__ bool bpe_warp_seg_min(uint16_t *segmin, uint32_t sg, 
     return __any_sync(FULL, valid && rk != BPE_INF);
 }
 
-// dynamic shared memory layout: sym[2][cap] rnk[2][cap] seg[2][cap] src[cap] segmin[2][cap+2], all uint16.
+// dynamic shared memory layout: sym[2][cap] rnk[2][cap] seg[2][cap] src[cap] segmin[2][cap+2] origin[cap]
+// segstart[cap], all uint16.  A segment none of whose pairs has a rule any more is finished: the next compaction pass
+// writes its tokens to tmp_tok at the segment's own place in the read (the rest of its span stays SYM_HOLE) and drops
+// it from the working sequence, so late rounds only touch the few long segments that are still merging.
 // One round = compaction pass (one barrier per chunk of BPE_NT symbols) -> barrier -> rank pass, which also collects
 // the next round's per-segment minima into the other segmin buffer -> barrier.
 __global__ void __launch_bounds__(BPE_NT) bpe_reads_kernel(const __grid_constant__ BpeArgs A) {
     extern __shared__ __align__(16) uint16_t sh[];
     __shared__ __align__(16) int warp_tmp[2][BPE_NT / 32];
-    __shared__ int s_any[2];
     const int cap = A.cap, tid = threadIdx.x;
     uint16_t *symb[2] = {sh, sh + cap};
     uint16_t *rnkb[2] = {sh + 2 * cap, sh + 3 * cap};
     uint16_t *segb[2] = {sh + 4 * cap, sh + 5 * cap};
     uint16_t *src = sh + 6 * cap;
     uint16_t *sminb[2] = {sh + 7 * cap, sh + 8 * cap + 2};
+    uint16_t *origin = sh + 9 * cap + 4;       // [cap] position in the read of each segment's first symbol
+    uint16_t *segstart = sh + 10 * cap + 4;    // [cap] index in the current sequence of each segment's first symbol
+    __shared__ int s_cnt;
     int pp = 0;
 
     for (int64_t r = blockIdx.x; r < A.n_rec; r += gridDim.x) {
@@ -136,7 +142,8 @@ __global__ void __launch_bounds__(BPE_NT) bpe_reads_kernel(const __grid_constant
             symb[0][i] = (uint16_t)(c < CLS_N ? c : (c == CLS_N ? SYM_N : SYM_UNK));
         }
         for (int i = tid; i <= n; i += BPE_NT) sminb[0][i] = (uint16_t)BPE_INF;     // at most n segments
-        if (tid == 0) { s_any[0] = 0; }
+        for (int i = tid; i < n; i += BPE_NT) A.tmp_tok[k0 + i] = (uint16_t)SYM_HOLE;
+        if (tid == 0) s_cnt = 0;
         __syncthreads();
         int seg_base = 0;
         for (int base = 0; base < n; base += BPE_NT) {       // chunked so the scan carries across chunks
@@ -153,22 +160,21 @@ __global__ void __launch_bounds__(BPE_NT) bpe_reads_kernel(const __grid_constant
             if (i < n) {
                 sg = (uint32_t)(seg_base + ex + start - 1);
                 segb[0][i] = (uint16_t)sg;
+                if (start) { origin[sg] = (uint16_t)i; segstart[sg] = (uint16_t)i; }
                 rk = (i + 1 < n) ? bpe_rank(A, symb[0][i], symb[0][i + 1]) : BPE_INF;
                 rnkb[0][i] = (uint16_t)rk;
             }
-            if (bpe_warp_seg_min(sminb[0], sg, rk, i < n) && (tid & 31) == 0) s_any[0] = 1;
+            bpe_warp_seg_min(sminb[0], sg, rk, i < n);
             seg_base += tot;
         }
         __syncthreads();
 
         // ---- rounds ----------------------------------------------------------------------
-        for (;;) {
-            if (!s_any[ms]) break;
+        while (n > 0) {
             uint16_t *sym = symb[cur], *rnk = rnkb[cur], *seg = segb[cur], *segmin = sminb[ms];
             uint16_t *sym2 = symb[cur ^ 1], *rnk2 = rnkb[cur ^ 1], *seg2 = segb[cur ^ 1], *smin2 = sminb[ms ^ 1];
             // the other minima buffer gets ready for the rank pass of this round
             for (int i = tid; i <= seg_base; i += BPE_NT) smin2[i] = (uint16_t)BPE_INF;
-            if (tid == 0) s_any[ms ^ 1] = 0;
             // flags, run parity, compaction
             int carry = 0;
             for (int base = 0; base < n; base += BPE_NT) {
@@ -188,47 +194,50 @@ __global__ void __launch_bounds__(BPE_NT) bpe_reads_kernel(const __grid_constant
                     // one look at the symbol's own pair; the run of selected pairs in front of it comes from the warp's
                     // ballot, and only a run that reaches the warp's first lane is followed back through shared memory
                     const int ln = tid & 31;
-                    const bool f = i < n && fires(i);
+                    // a finished segment leaves: its tokens go to their place in the read
+                    const uint32_t sgi = i < n ? (uint32_t)seg[i] : 0u;
+                    const bool fin = i < n && segmin[sgi] == BPE_INF;
+                    if (fin) A.tmp_tok[k0 + origin[sgi] + (i - (int)segstart[sgi])] = sym[i];
+                    const uint32_t fb = __ballot_sync(0xffffffffu, fin);
+                    if (ln == 0 && fb) atomicAdd(&s_cnt, __popc(fb));
+                    const bool f = i < n && !fin && fires(i);
                     const uint32_t Fw = __ballot_sync(0xffffffffu, f);
                     int c = ln ? __clz(~(Fw << (32 - ln))) : 0;  // selected pairs directly in front, inside the warp
                     if (c > ln) c = ln;
                     if (f && c == ln) { int j = i - ln - 1; while (j >= 0 && fires(j)) { ++c; --j; } }
                     merge = f && (c & 1) == 0;
                     const bool pm = __shfl_up_sync(0xffffffffu, merge, 1);
-                    if (i < n) keep = !(ln ? pm : (i > 0 && merges(i - 1)));
+                    if (i < n && !fin) keep = !(ln ? pm : (i > 0 && merges(i - 1)));
                 }
                 int tot;
                 int w = carry + bpe_exscan(keep, warp_tmp, pp, tot);
                 if (keep) {
                     sym2[w] = merge ? (uint16_t)(4u + rnk[i]) : sym[i];
                     seg2[w] = seg[i];
+                    if (i == 0 || seg[i - 1] != seg[i]) segstart[seg[i]] = (uint16_t)w;   // first symbol of its segment
                     src[w] = (uint16_t)(merge ? 0xffffu : i);    // 0xffff: freshly merged token
                 }
                 carry += tot;
             }
             __syncthreads();
             const int n2 = carry;
-            bool any = false;
             for (int base = 0; base < n2; base += BPE_NT) {
                 const int w = base + tid;
                 uint32_t rk = BPE_INF, sg = 0;
                 if (w < n2) {
-                    if (w + 1 < n2) {
+                    if (w + 1 < n2 && seg2[w] == seg2[w + 1]) {      // neighbours of different segments never pair
                         if (src[w] == 0xffffu || src[w + 1] == 0xffffu) rk = bpe_rank(A, sym2[w], sym2[w + 1]);
                         else rk = rnk[src[w]];
                     }
                     rnk2[w] = (uint16_t)rk;
                     sg = seg2[w];
                 }
-                any |= bpe_warp_seg_min(smin2, sg, rk, w < n2);
+                bpe_warp_seg_min(smin2, sg, rk, w < n2);
             }
-            if (any && (tid & 31) == 0) s_any[ms ^ 1] = 1;
             n = n2; cur ^= 1; ms ^= 1;
             __syncthreads();
         }
-        // ---- write token numbers --------------------------------------------------------
-        for (int i = tid; i < n; i += BPE_NT) A.tmp_tok[k0 + i] = symb[cur][i];
-        if (tid == 0) A.tok_cnt[r] = n;
+        if (tid == 0) A.tok_cnt[r] = s_cnt;     // every token has been written by the pass that retired its segment
     }
 }
 
@@ -257,21 +266,30 @@ __global__ void __launch_bounds__(1024) scan_counts_kernel(const int32_t *cnt, i
     if (tid == 0) out_off[n] = s_carry;
 }
 
+// ids of read r = its tmp_tok entries that are not holes, in order (one warp per read)
 template <typename IdT>
 __global__ void __launch_bounds__(256) bpe_gather_kernel(const uint16_t *tmp_tok, const int64_t *koff,
                                                          const int64_t *out_off, int64_t n_rec, IdT *ids,
                                                          int64_t ids_cap, int32_t base_id, int32_t n_id,
                                                          int32_t unk_id, uint32_t *status) {
+    constexpr uint32_t FULL = 0xffffffffu;
     const int lane = threadIdx.x & 31;
     const int64_t warp = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
     const int64_t nwarps = ((int64_t)gridDim.x * blockDim.x) >> 5;
     for (int64_t r = warp; r < n_rec; r += nwarps) {
-        const int64_t k0 = koff[r], o0 = out_off[r];
-        const int n = (int)(out_off[r + 1] - o0);
-        for (int i = lane; i < n; i += 32) {
-            uint32_t s = tmp_tok[k0 + i];
-            int32_t id = s == SYM_N ? n_id : (s == SYM_UNK ? unk_id : (int32_t)(base_id + s));
-            if (o0 + i < ids_cap) ids[o0 + i] = (IdT)id; else status[0] = 1u;
+        const int64_t k0 = koff[r], o_end = out_off[r + 1];
+        const int n = (int)(koff[r + 1] - k0);
+        int64_t o = out_off[r];
+        for (int base = 0; base < n && o < o_end; base += 32) {
+            const int i = base + lane;
+            const uint32_t s = i < n ? (uint32_t)tmp_tok[k0 + i] : SYM_HOLE;
+            const uint32_t vm = __ballot_sync(FULL, s != SYM_HOLE);
+            const int64_t at = o + __popc(vm & ((1u << lane) - 1u));
+            if (s != SYM_HOLE && at < o_end) {               // (a read that did not fit the workspace has no tokens)
+                const int32_t id = s == SYM_N ? n_id : (s == SYM_UNK ? unk_id : (int32_t)(base_id + s));
+                if (at < ids_cap) ids[at] = (IdT)id; else status[0] = 1u;
+            }
+            o += __popc(vm);
         }
     }
 }

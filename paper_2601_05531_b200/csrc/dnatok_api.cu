@@ -225,7 +225,7 @@ int ctx_reserve_bpe(dnatok_t *h, EncCtx &c, int64_t n_bytes, int64_t n_rec, cuda
     return DNATOK_OK;
 }
 
-size_t bpe_smem_bytes(int cap) { return (size_t)(9 * cap + 8) * sizeof(uint16_t); }
+size_t bpe_smem_bytes(int cap) { return (size_t)(11 * cap + 8) * sizeof(uint16_t); }
 
 int encode_on(dnatok_t *h, EncCtx &c, const uint8_t *d_bytes, int64_t n_bytes, const int64_t *d_rec_off,
               int64_t n_rec, int64_t off_bias, void *d_ids, int64_t ids_cap, int64_t *d_out_off, cudaStream_t st) {
