@@ -54,7 +54,7 @@ def workload_spec(config: int, scale: float = 1.0, k: int = 6) -> dict:
     if config == 4:
         n = max(1, int(65536 * scale))
         return dict(name=f"config4: BPE 4,092 merges, {n} reads of 500-1,500 bases, 2% N, int32",
-                    gen=("config4", dict(n_reads=n)), tok=dict(mode="bpe", max_record_bytes=2048), seq_len=0)
+                    gen=("config4", dict(n_reads=n)), tok=dict(mode="bpe", max_record_bytes=1536), seq_len=0)
     if config == 5:
         tb = int((8 << 30) * scale)
         return dict(name=f"config5: streaming {tb} bytes pinned, 64 MiB chunks x 4 streams, 6-mer + pad 8192 + mask",

@@ -433,8 +433,8 @@ int dnatok_create(const dnatok_config *cfg_in, int device, dnatok_t **out) {
         if (cudaMalloc(&h->d_table, table.size() * sizeof(uint64_t)) != cudaSuccess) return bail(DNATOK_ENOMEM);
         if (cudaMemcpy(h->d_table, table.data(), table.size() * sizeof(uint64_t), cudaMemcpyHostToDevice) != cudaSuccess)
             return bail(DNATOK_ECUDA);
-        int cap = 256;
-        while (cap < cfg.max_record_bytes && cap < 8192) cap <<= 1;
+        // per-read workspace: the smaller it is, the more reads are in flight per SM, and that is what sets the rate
+        int cap = (int)std::min<int64_t>(8192, std::max<int64_t>(256, (cfg.max_record_bytes + 63) & ~(int64_t)63));
         h->bpe_cap = cap;
         if (cudaFuncSetAttribute(bpe_reads_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                  (int)bpe_smem_bytes(cap)) != cudaSuccess) return bail(DNATOK_ECUDA);
