@@ -176,6 +176,14 @@ int64_t dnatok_launch_count(const dnatok_t *h);
  */
 int dnatok_set_super_tile(dnatok_t *h, int32_t sub_tiles);
 
+/*
+ * Tuning / test knob: cap on the number of persistent CTAs the encode, BPE and pad kernels launch (0 = the
+ * default, one grid's worth of resident CTAs).  Tests set 1, 2, 7 so that one CTA walks many super-tiles /
+ * reads and every buffer-reuse path of the persistent kernels runs deterministically on small inputs.
+ * Results never depend on it.  EINVAL if max_ctas < 0.
+ */
+int dnatok_set_grid_cap(dnatok_t *h, int32_t max_ctas);
+
 /* Library version string, e.g. "dnatok-b200 0.1 (sm_100a)".                                            */
 const char *dnatok_version(void);
 

@@ -25,7 +25,7 @@ __all__ = [
     "DNATok", "Config", "Batch", "DNATokError", "lib", "library_path",
     "SINGLE_NT", "KMER", "BPE", "I16", "I32", "TAIL_PER_BASE", "TAIL_DROP", "TAIL_UNK", "PAD_LEFT", "PAD_RIGHT",
     "dnatok_create", "dnatok_destroy", "dnatok_encode", "dnatok_pad", "dnatok_stream_encode", "dnatok_check",
-    "dnatok_last_error", "dnatok_launch_count", "dnatok_version", "dnatok_config_default", "dnatok_set_super_tile",
+    "dnatok_last_error", "dnatok_launch_count", "dnatok_version", "dnatok_config_default", "dnatok_set_super_tile", "dnatok_set_grid_cap",
 ]
 
 SINGLE_NT, KMER, BPE = 0, 1, 2
@@ -65,6 +65,7 @@ class _CBatch(ctypes.Structure):
 _BATCH_FN = ctypes.CFUNCTYPE(None, ctypes.c_void_p, ctypes.POINTER(_CBatch))
 _lib = None
 SUPER_TILE = 0      # sub-tiles per super-tile applied to new DNATok handles (0 = automatic); a tuning knob, see dnatok.h
+GRID_CAP = 0        # cap on persistent CTAs per launch applied to new DNATok handles (0 = none); a test knob, see dnatok.h
 
 
 def library_path() -> str:
@@ -104,6 +105,8 @@ def lib() -> ctypes.CDLL:
         L.dnatok_last_error.argtypes = [vp]
         L.dnatok_set_super_tile.restype = ctypes.c_int
         L.dnatok_set_super_tile.argtypes = [vp, i32]
+        L.dnatok_set_grid_cap.restype = ctypes.c_int
+        L.dnatok_set_grid_cap.argtypes = [vp, i32]
         L.dnatok_launch_count.restype = i64
         L.dnatok_launch_count.argtypes = [vp]
         _lib = L
@@ -165,6 +168,10 @@ def dnatok_last_error(h: int) -> str:
 
 def dnatok_set_super_tile(h: int, sub_tiles: int) -> None:
     _chk(h, lib().dnatok_set_super_tile(h, int(sub_tiles)))
+
+
+def dnatok_set_grid_cap(h: int, max_ctas: int) -> None:
+    _chk(h, lib().dnatok_set_grid_cap(h, int(max_ctas)))
 
 
 def dnatok_launch_count(h: int) -> int:
@@ -263,6 +270,8 @@ class DNATok:
         self.h = dnatok_create(c, device)
         if SUPER_TILE:
             dnatok_set_super_tile(self.h, SUPER_TILE)
+        if GRID_CAP:
+            dnatok_set_grid_cap(self.h, GRID_CAP)
         self.id_torch_dtype = torch.int16 if self.cfg.id_dtype == I16 else torch.int32
 
     def close(self) -> None:

@@ -73,6 +73,7 @@ struct dnatok {
     StreamRing ring;
     int enc_ctas_per_sm = 1, bpe_ctas_per_sm = 1;
     int force_S = 0;                   // dnatok_set_super_tile: fixed super-tile size in sub-tiles (0 = automatic)
+    int grid_cap = 0;                  // dnatok_set_grid_cap: at most this many persistent CTAs per launch (0 = no cap)
     int64_t launches = 0;
     std::string err;
 };
@@ -181,6 +182,7 @@ int launch_tiles(dnatok_t *h, EncCtx &c, const EncParams &prm, const uint8_t *d_
     a.lut = h->d_lut; a.descs = c.descs; a.ls = c.ls; a.rec_k = c.rec_k; a.first_rec = c.first_rec; a.ticket = c.ticket; a.ticket_base = c.ticket_base;
     a.status = c.d_status; a.gen = c.gen; a.n_tiles = (int32_t)n_tiles; a.prm = prm;
     int grid = (int)std::min<int64_t>(n_tiles, (int64_t)h->sm_count * h->enc_ctas_per_sm);
+    if (h->grid_cap > 0) grid = std::min(grid, h->grid_cap);
     tile_first_rec_kernel<<<(unsigned)((n_tiles + 1 + 255) / 256), 256, 0, st>>>(a);
     CU(cudaGetLastError());
     // the headline shapes get a kernel with only their own emission variant compiled in (smaller instruction footprint)
@@ -248,6 +250,7 @@ int encode_on(dnatok_t *h, EncCtx &c, const uint8_t *d_bytes, int64_t n_bytes, c
         b.cls = c.cls; b.koff = c.koff; b.n_rec = n_rec; b.table = h->d_table; b.table_mask = h->table_mask;
         b.cap = h->bpe_cap; b.tmp_tok = c.tmp_tok; b.tok_cnt = c.tok_cnt; b.status = c.d_status;
         int grid = (int)std::min<int64_t>(n_rec, (int64_t)h->sm_count * h->bpe_ctas_per_sm);
+        if (h->grid_cap > 0) grid = std::min(grid, h->grid_cap);
         bpe_reads_kernel<<<grid, BPE_NT, bpe_smem_bytes(h->bpe_cap), st>>>(b);
         CU(cudaGetLastError());
         h->launches += 1;
@@ -257,6 +260,7 @@ int encode_on(dnatok_t *h, EncCtx &c, const uint8_t *d_bytes, int64_t n_bytes, c
     h->launches += 1;
     if (n_rec > 0) {
         int grid = (int)std::min<int64_t>((n_rec + 7) / 8, (int64_t)h->sm_count * 8);
+        if (h->grid_cap > 0) grid = std::min(grid, h->grid_cap);
         if (cfg.id_dtype == DNATOK_I16)
             bpe_gather_kernel<int16_t><<<grid, 256, 0, st>>>(c.tmp_tok, c.koff, d_out_off, n_rec, (int16_t *)d_ids, ids_cap,
                                                            cfg.base_id, cfg.n_id, cfg.unk_id, c.d_status);
@@ -276,6 +280,7 @@ int pad_on(dnatok_t *h, const void *d_ids, const int64_t *d_out_off, int64_t n_r
     a.ids = d_ids; a.out_off = d_out_off; a.n_rows = n_rec; a.batch_ids = d_batch; a.mask = d_mask;
     a.seq_len = h->cfg.seq_len; a.pad_side = h->cfg.pad_side; a.pad_id = h->cfg.pad_id;
     int grid = (int)std::min<int64_t>(n_rec, (int64_t)h->sm_count * 16);
+    if (h->grid_cap > 0) grid = std::min(grid, h->grid_cap);
     if (h->cfg.id_dtype == DNATOK_I16) pad_rows_kernel<int16_t><<<grid, 256, 0, st>>>(a);
     else pad_rows_kernel<int32_t><<<grid, 256, 0, st>>>(a);
     CU(cudaGetLastError());
@@ -599,6 +604,13 @@ int dnatok_set_super_tile(dnatok_t *h, int32_t sub_tiles) {
     if (!h) return DNATOK_EINVAL;
     if (sub_tiles < 0 || sub_tiles > S_MAX) return fail(h, DNATOK_EINVAL, "dnatok_set_super_tile: sub_tiles must be in 0..%d", S_MAX);
     h->force_S = sub_tiles;
+    return DNATOK_OK;
+}
+
+int dnatok_set_grid_cap(dnatok_t *h, int32_t max_ctas) {
+    if (!h) return DNATOK_EINVAL;
+    if (max_ctas < 0) return fail(h, DNATOK_EINVAL, "dnatok_set_grid_cap: max_ctas must be >= 0");
+    h->grid_cap = max_ctas;
     return DNATOK_OK;
 }
 
