@@ -37,8 +37,26 @@ MIB = 1 << 20
 
 
 # ----------------------------------------------------------------------------------------- workloads
-def workload_spec(config: int, scale: float = 1.0, k: int = 6) -> dict:
+def dense_lut() -> np.ndarray:
+    """The default byte -> class table with no SKIP class ('\\n', '\\r' -> UNK): together with strip_headers = 0 this
+    is the create-time spec of the no-scan encoder (kept bases = bytes).  Configs 2 and 4 hold no newline and no
+    header, so their result is the same under either table; the oracle is given the same table."""
+    lut = np.full(256, 5, dtype=np.uint8)
+    for i, (u, l) in enumerate(zip(b"ACGTN", b"acgtn")):
+        lut[u] = lut[l] = i
+    return lut
+
+
+def workload_spec(config: int, scale: float = 1.0, k: int = 6, dense: bool = True) -> dict:
     """Binding-style kwargs + generator call for BASELINE.json configs[config-1]."""
+    spec = _workload_spec(config, scale, k)
+    if dense and config in (2, 4):
+        spec["tok"].update(class_lut=dense_lut(), strip_headers=False)
+        spec["name"] += ", dense spec (no SKIP class, strip_headers 0)"
+    return spec
+
+
+def _workload_spec(config: int, scale: float = 1.0, k: int = 6) -> dict:
     if config == 1:
         return dict(name="config1: single-nt, 16 x 65,536 bases, 60-col lines, 1% N, 5% lowercase",
                     gen=("config1", {}), tok=dict(mode="single_nt"), seq_len=0)
@@ -76,7 +94,11 @@ def oracle_config(spec: dict, w):
     import oracle
     t = spec["tok"]
     m = {"single_nt": oracle.SINGLE_NT, "kmer": oracle.KMER, "bpe": oracle.BPE}[t["mode"]]
-    return oracle.Config(mode=m, k=t.get("k", 1), merges=w.merges, seq_len=spec["seq_len"])
+    kw = {}
+    if t.get("class_lut") is not None:
+        kw["class_lut"] = np.asarray(t["class_lut"], dtype=np.uint8)
+    return oracle.Config(mode=m, k=t.get("k", 1), merges=w.merges, seq_len=spec["seq_len"],
+                         strip_headers=bool(t.get("strip_headers", True)), **kw)
 
 
 # ----------------------------------------------------------------------------------------- clocks
@@ -198,7 +220,7 @@ def run_reference(args) -> None:
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    spec = workload_spec(args.config, args.scale, args.k)
+    spec = workload_spec(args.config, args.scale, args.k, not args.no_dense)
     w = generate(spec, seed=0)
     data, offs, bases = oracle_sample(w)
     cfg = oracle_config(spec, w)
@@ -266,7 +288,7 @@ def run_ours(args) -> None:
         dist.all_reduce(t, op=dist.ReduceOp.SUM)
         return float(t.item())
 
-    spec = workload_spec(args.config, args.scale, args.k)
+    spec = workload_spec(args.config, args.scale, args.k, not args.no_dense)
     tokkw = dict(spec["tok"])
     # ---- input: generated straight into pinned host memory (also the e2e source) ------------------
     t0 = time.perf_counter()
@@ -331,7 +353,7 @@ def run_ours(args) -> None:
     launches = tok.launch_count - launches0
     tok.check()
     ms_per_step = max_over_ranks(total_ms / args.steps)
-    launches_per_step = (2 if tokkw["mode"] != "bpe" else 5) + (1 if L else 0)   # pre-pass + encode (+ BPE passes) (+ pad)
+    launches_per_step = (2 if tokkw["mode"] != "bpe" else 5) + (1 if L else 0) + (1 if tok.cfg.class_lut is not None else 0)   # pre-pass + encode (+ BPE passes) (+ pad)
     assert launches >= launches_per_step * args.steps
 
     # ---- parity on sampled records against the oracle (untimed) -----------------------------------
@@ -459,6 +481,7 @@ def main() -> None:
     ap.add_argument("--traffic", type=float, default=None,
                     help="ncu dram read+write bytes per launch of the dominant kernel (from profiles/)")
     ap.add_argument("--super-tile", type=int, default=0, help="tuning: sub-tiles per super-tile (0 = automatic)")
+    ap.add_argument("--no-dense", action="store_true", help="configs 2 and 4: default table (with SKIP) instead of the dense spec")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--no-parity", action="store_true")

@@ -77,12 +77,14 @@ struct EncArgs {
     int64_t out_bias;             // added to every out_off value and id position (0)
     const uint8_t *lut;           // [256] device
     TileDesc *descs;              // [n_tiles]
+    TileDesc *gdescs;             // [n_tiles / 32 + 1] group aggregates (a0 / a1 only) of the two-level look-back
     uint32_t *ls;                 // [n_tiles] line-state chain words
     int64_t *first_rec;           // [n_tiles + 1]: first r in [0, n_rec] whose position is >= tile * S * TB (n_rec + 1 if none)
     int32_t *rec_k;               // [n_rec + 1] scratch: kept bases of the super-tile before each record start (many-starts path)
     unsigned long long *ticket;   // tile ticket counter
     unsigned long long ticket_base;
     uint32_t *status;             // device-mapped host status word
+    unsigned long long *prof;     // phase timers (debug builds with -DDTK_PROF only)
     uint32_t gen;
     int32_t n_tiles;              // super-tiles
     int32_t S;                    // sub-tiles per super-tile (1..S_MAX)

@@ -24,6 +24,7 @@ namespace {
 // scan scratch of one in-flight encode: tile descriptors, ticket counter, host-mapped status words
 struct EncCtx {
     TileDesc *descs = nullptr;
+    TileDesc *gdescs = nullptr;        // [descs_cap / 32 + 2] group aggregates of the two-level look-back
     uint32_t *ls = nullptr;            // [descs_cap] line-state chain words
     int64_t *first_rec = nullptr;      // [descs_cap + 1] record range of every super-tile (pre-pass output)
     int64_t descs_cap = 0;
@@ -34,6 +35,7 @@ struct EncCtx {
     uint32_t *h_status = nullptr;      // pinned + mapped: [0] capacity overflow, [1] scan protocol failure
     uint32_t *d_status = nullptr;      // device alias of h_status
     uint32_t gen = 0;
+    unsigned long long *prof = nullptr;   // phase timers of debug builds (-DDTK_PROF)
     // BPE pass scratch
     uint8_t *cls = nullptr;  int64_t cls_cap = 0;
     uint16_t *tmp_tok = nullptr;
@@ -116,11 +118,14 @@ int ctx_init(dnatok_t *h, EncCtx &c) {
     CU(cudaHostAlloc(&c.h_status, 2 * sizeof(uint32_t), cudaHostAllocMapped));
     c.h_status[0] = c.h_status[1] = 0;
     CU(cudaHostGetDevicePointer((void **)&c.d_status, c.h_status, 0));
+    CU(cudaMalloc(&c.prof, 64 * sizeof(unsigned long long)));
+    CU(cudaMemset(c.prof, 0, 64 * sizeof(unsigned long long)));
     return DNATOK_OK;
 }
 
 void ctx_free(EncCtx &c) {
-    cudaFree(c.descs); cudaFree(c.ls); cudaFree(c.first_rec); cudaFree(c.rec_k); cudaFree(c.ticket); cudaFreeHost(c.h_status);
+    cudaFree(c.descs); cudaFree(c.gdescs); cudaFree(c.ls); cudaFree(c.first_rec); cudaFree(c.rec_k); cudaFree(c.ticket); cudaFreeHost(c.h_status);
+    cudaFree(c.prof);
     cudaFree(c.cls); cudaFree(c.tmp_tok); cudaFree(c.koff); cudaFree(c.tok_cnt);
     c = EncCtx();
 }
@@ -137,10 +142,13 @@ int ctx_reserve_tiles(dnatok_t *h, EncCtx &c, int64_t n_tiles, int64_t n_rec, cu
     if (n_tiles <= c.descs_cap) return DNATOK_OK;
     int64_t cap = std::max<int64_t>(n_tiles + n_tiles / 4, 1024);
     if (c.descs) CU(cudaFreeAsync(c.descs, st));
+    if (c.gdescs) CU(cudaFreeAsync(c.gdescs, st));
     if (c.ls) CU(cudaFreeAsync(c.ls, st));
     if (c.first_rec) CU(cudaFreeAsync(c.first_rec, st));
-    c.descs = nullptr; c.ls = nullptr; c.first_rec = nullptr; c.descs_cap = 0;
+    c.descs = nullptr; c.gdescs = nullptr; c.ls = nullptr; c.first_rec = nullptr; c.descs_cap = 0;
     CU(cudaMallocAsync((void **)&c.descs, (size_t)cap * sizeof(TileDesc), st));
+    CU(cudaMallocAsync((void **)&c.gdescs, (size_t)(cap / 32 + 2) * sizeof(TileDesc), st));
+    CU(cudaMemsetAsync(c.gdescs, 0, (size_t)(cap / 32 + 2) * sizeof(TileDesc), st));
     CU(cudaMallocAsync((void **)&c.ls, (size_t)cap * sizeof(uint32_t), st));
     CU(cudaMallocAsync((void **)&c.first_rec, (size_t)(cap + 1) * sizeof(int64_t), st));
     CU(cudaMemsetAsync(c.descs, 0, (size_t)cap * sizeof(TileDesc), st));
@@ -152,6 +160,7 @@ int ctx_reserve_tiles(dnatok_t *h, EncCtx &c, int64_t n_tiles, int64_t n_rec, cu
 int ctx_next_gen(dnatok_t *h, EncCtx &c, cudaStream_t st) {
     if (++c.gen >= (1u << 24) - 1) {       // generation tags are 24 bits wide in TileDesc::l_word
         if (c.descs) CU(cudaMemsetAsync(c.descs, 0, (size_t)c.descs_cap * sizeof(TileDesc), st));
+        if (c.gdescs) CU(cudaMemsetAsync(c.gdescs, 0, (size_t)(c.descs_cap / 32 + 2) * sizeof(TileDesc), st));
         if (c.ls) CU(cudaMemsetAsync(c.ls, 0, (size_t)c.descs_cap * sizeof(uint32_t), st));
         c.gen = 1;
     }
@@ -200,8 +209,8 @@ int launch_tiles(dnatok_t *h, EncCtx &c, const EncParams &prm, const uint8_t *d_
     rc = ctx_next_gen(h, c, st); if (rc) return rc;
     a.rec_off = d_rec_off; a.n_rec = n_rec; a.off_bias = off_bias;
     a.ids = ids; a.ids_cap = ids_cap; a.out_off = out_off; a.out_bias = 0;
-    a.lut = h->d_lut; a.descs = c.descs; a.ls = c.ls; a.rec_k = c.rec_k; a.first_rec = c.first_rec; a.ticket = c.ticket; a.ticket_base = c.ticket_base;
-    a.status = c.d_status; a.gen = c.gen; a.n_tiles = (int32_t)n_tiles; a.prm = prm;
+    a.lut = h->d_lut; a.descs = c.descs; a.gdescs = c.gdescs; a.ls = c.ls; a.rec_k = c.rec_k; a.first_rec = c.first_rec; a.ticket = c.ticket; a.ticket_base = c.ticket_base;
+    a.status = c.d_status; a.prof = c.prof; a.gen = c.gen; a.n_tiles = (int32_t)n_tiles; a.prm = prm;
     int grid = (int)std::min<int64_t>(n_tiles, slots);
     if (h->grid_cap > 0) grid = std::min(grid, h->grid_cap);
     tile_first_rec_kernel<<<(unsigned)((n_tiles + 1 + 255) / 256), 256, 0, st>>>(a);
@@ -633,6 +642,16 @@ int dnatok_set_grid_cap(dnatok_t *h, int32_t max_ctas) {
     h->grid_cap = max_ctas;
     return DNATOK_OK;
 }
+
+#ifdef DTK_PROF
+// debug builds only: read and clear the phase timers of the handle's resident-encode context
+int dnatok_debug_prof(dnatok_t *h, unsigned long long *out64) {
+    cudaDeviceSynchronize();
+    cudaMemcpy(out64, h->ctx.prof, 64 * sizeof(unsigned long long), cudaMemcpyDeviceToHost);
+    cudaMemset(h->ctx.prof, 0, 64 * sizeof(unsigned long long));
+    return DNATOK_OK;
+}
+#endif
 
 const char *dnatok_last_error(const dnatok_t *h) { return h ? h->err.c_str() : "null handle"; }
 

@@ -46,7 +46,7 @@ constexpr int SW_ALL = SW_CODE + SW_FLAG;    // multiple of 4 words
 constexpr int EV_MAX = 64;                   // record starts per tile handled through the shared-memory tables
 constexpr int NSE = EV_MAX + NWC;            // segment-table entries: entry 0, the record starts, 7 region starts
 constexpr uint32_t LS_UNKNOWN = 3;
-enum : int { BAR_PREP = 1, BAR_DONE = 2, BAR_READY = 3 };   // READY alternates between ids 3 and 4
+enum : int { BAR_PREP = 1, BAR_READY = 3 };   // PREP alternates between ids 1 and 2, READY between 3 and 4; DONE is a polled counter
 
 struct TileAgg {                             // aggregate of one tile, kept until its look-back
     int32_t fk, lk, closed, tn;              // kept before first / after last record start, tokens of records inside, tail classes held
@@ -60,9 +60,7 @@ struct TileCtl {                             // scan warp -> compute warps, one 
     int32_t emit;                            // after the compaction: emit the tile held in buffer emit_buf
     int32_t emit_buf;
     int32_t emit_generic;                    // that tile has more record starts than the tables hold
-    int32_t redo;                            // region entry line states are given in ent_ls (second pass over a tile)
     int32_t last;                            // leave the loop after this iteration
-    uint32_t ent_ls[NWC];
 };
 
 struct TileBuf {                             // per stream buffer
@@ -74,7 +72,10 @@ struct TileBuf {                             // per stream buffer
     int32_t ktot, ntok;                      // kept bases, tokens
     int32_t pend, tok0, nwin0;               // entry 0: carried bases, its tokens, its windows
     int32_t cum[NWC + 1];                    // kept bases before each region
+    int32_t rbase[NWC];                      // stream slot of each region's first kept base (reg_slot + what was dropped)
     int32_t reg_cnt[NWC];
+    int32_t reg_hfix[NWC];                   // kept bases in front of the region's first line reset (dropped if the
+                                             //   region turns out to have started inside a header line)
     uint32_t reg_ls[NWC];                    // known << 8 | entry << 4 | hr << 2 | x   (region line-state record)
     int32_t reg_e0[NWC + 1];                 // segment-table range of each region
     uint16_t ev_p[EV_MAX];                   // tile positions of the record starts
@@ -87,11 +88,12 @@ struct TileBuf {                             // per stream buffer
 struct Smem7 {
     uint32_t strm[2][SW_ALL];                // per buffer -- code stream: slot u at word u>>4, bits 31-2(u&15), 30-2(u&15);
                                              // flag stream at + SW_CODE: slot u at word u>>5, bit 31-(u&31)
-    uint4 stage[NWC][128];                   // per compute warp: the lanes' raw 64 bytes (16-byte chunks XOR-swizzled)
+    uint4 stage[NWC][128];                   // per compute warp: the lanes' raw 64 bytes
     unsigned long long wk[NWC][32];          // per compute warp: record-start bitmap, then keep masks (event steps only)
     uint16_t offw[NWC][32];
     TileBuf tb[2];
     TileCtl ctl[2];
+    int32_t done_cnt;                        // regions compacted since the kernel started (compute warps -> scan warp)
     uint8_t lut[256];
 };
 static_assert(sizeof(Smem7) <= 76288, "three CTAs per SM (227 KiB, 1 KiB reserved per CTA)");
@@ -127,7 +129,7 @@ __device__ __forceinline__ int slot_of(const TileBuf &tb, int u) {
     int r = 0;
 #pragma unroll
     for (int w = 1; w < NWC; ++w) r += (u >= tb.cum[w]) ? 1 : 0;
-    return reg_slot(r) + (u - tb.cum[r]);
+    return tb.rbase[r] + (u - tb.cum[r]);
 }
 
 template <typename IdT>
@@ -536,80 +538,127 @@ __global__ void __launch_bounds__(DS_NT) dense_offsets_kernel(const __grid_const
 }
 
 // ---- look-back (scan warp): everything before tile `tile` -------------------------------------------------------
-// Windows of 32 predecessors, nearest first.  Lane l of a window holds tile base - l: an aggregate, an inclusive
-// prefix, or nothing yet (then the warp polls).  A window with an inclusive prefix at lane f ends the walk: lanes
-// < f extend it.  A window of 32 aggregates is folded into the running aggregate of the nearer tiles.
-__device__ __noinline__ Pre look_back(const EncArgs &A, int tile, int lane) {
+// Two levels.  Tiles form groups of 32; the scan warp of a group's last tile publishes the GROUP aggregate (all 32
+// tile aggregates folded) as soon as it has seen them, and that tile's inclusive prefix is the group's inclusive
+// prefix.  A look-back is then: one window over the predecessors inside the tile's own group, and windows of 32
+// GROUPS (1024 tiles each) from there on -- two reads in practice, however many tiles are in flight.
+// Lane l of a window holds item base - l: an aggregate, an inclusive prefix, or nothing yet.  A window with an
+// inclusive prefix at lane f ends the walk: lanes < f extend it.  A window of aggregates only is folded into the
+// running aggregate of the nearer items.  ONE attempt: when a needed item has published nothing yet, `ready` comes
+// back false and the caller tries again later (the scan warp never blocks here).
+struct Win { uint4 a0, a1, i0, i1; uint32_t st; };
+
+// lanes < f of a window (aggregates; far = high lane) folded into one aggregate
+__device__ __forceinline__ Agg fold_window(const Win &w, int f, const EncParams &P, int lane) {
+    constexpr uint32_t FULL = 0xffffffffu;
+    const int k = P.k;
+    const bool in = lane < f;
+    const int fk_l = in ? (int)w.a0.y : 0, lk_l = (int)w.a0.z, cl_l = (int)(w.a0.w & 0x7fffffffu);
+    const bool ev_l = in && (w.a0.w >> 31);
+    int Ps = fk_l;                                       // kept-before-first-start summed over lanes >= this one
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) { const int t = __shfl_down_sync(FULL, Ps, d); if (lane + d < 32) Ps += t; }
+    const uint32_t evmask = __ballot_sync(FULL, ev_l);
+    const int P0 = __shfl_sync(FULL, Ps, 0);
+    Agg W; W.hasev = evmask != 0; W.closed = 0;
+    if (!evmask) { W.fk = P0; W.lk = P0; }
+    else {
+        const uint32_t higher = lane == 31 ? 0u : (evmask & ~((2u << lane) - 1u));
+        const int ep = higher ? __ffs(higher) - 1 : -1;              // next farther item with a record start
+        const int P_ep = __shfl_sync(FULL, Ps, ep < 0 ? 0 : ep), lk_ep = __shfl_sync(FULL, lk_l, ep < 0 ? 0 : ep);
+        int t32 = 0;
+        if (ev_l) t32 = cl_l + (ep >= 0 ? tok_count32(lk_ep + Ps - P_ep, P) : 0);
+        W.closed = __reduce_add_sync(FULL, t32);
+        const int e1 = 31 - __clz(evmask), e0 = __ffs(evmask) - 1;
+        W.fk = __shfl_sync(FULL, Ps, e1);
+        W.lk = __shfl_sync(FULL, lk_l, e0) + P0 - __shfl_sync(FULL, Ps, e0);
+    }
+    W.tn = 0; W.tail = 0;
+    if (P.mode == MODE_KMER && k > 1) {
+        const unsigned long long mytail = (unsigned long long)w.a1.z | ((unsigned long long)((w.a1.y >> 4) & 0x3ffu) << 32);
+        const int mycnt = (int)(w.a1.y & 15u);
+        const int want = min(k - 1, W.lk);
+        for (int l = 0; l < f && W.tn < want; ++l) {
+            const unsigned long long tl = __shfl_sync(FULL, mytail, l);
+            const int cn = min(__shfl_sync(FULL, mycnt, l), want - W.tn);
+            W.tail |= low_classes(tl, cn) << (3 * W.tn);
+            W.tn += cn;
+            if ((evmask >> l) & 1u) break;
+        }
+    }
+    return W;
+}
+// the inclusive prefix held by lane f of a window
+__device__ __forceinline__ Pre incl_at(const Win &w, int f) {
+    constexpr uint32_t FULL = 0xffffffffu;
+    Pre F;
+    const int64_t fT = (int64_t)(((uint64_t)w.i0.z << 32) | w.i0.y), fq = (int64_t)(((uint64_t)w.i1.z << 32) | w.i1.y);
+    const unsigned long long ftail = (unsigned long long)w.i1.w | ((unsigned long long)((w.i0.w >> 8) & 0x3ffu) << 32);
+    F.T = __shfl_sync(FULL, fT, f); F.o.q = __shfl_sync(FULL, fq, f);
+    const uint32_t fw = __shfl_sync(FULL, w.i0.w, f);
+    F.o.r = (int32_t)(fw & 15u); F.cnt = (int)((fw >> 4) & 15u);
+    F.tail = __shfl_sync(FULL, ftail, f);
+    return F;
+}
+__device__ __forceinline__ void publish_agg(TileDesc *D, uint32_t tagA, const Agg &g) {
+    st_vol128(&D->a0, make_uint4(tagA, (uint32_t)g.fk, (uint32_t)g.lk, (uint32_t)g.closed | ((uint32_t)(g.hasev != 0) << 31)));
+    st_vol128(&D->a1, make_uint4(tagA, (uint32_t)g.tn | ((uint32_t)(g.tail >> 32) << 4), (uint32_t)g.tail, 0u));
+}
+
+// own: the tile's own aggregate (the last tile of a group folds it into the group aggregate it publishes)
+__device__ __noinline__ Pre look_back(const EncArgs &A, int tile, const Agg &own, int lane, bool force, bool &ready) {
     constexpr uint32_t FULL = 0xffffffffu;
     const EncParams &P = A.prm;
-    const int k = P.k;
     const uint32_t tagA = (A.gen << 2) | ST_AGG, tagI = (A.gen << 2) | ST_INCL;
-    Agg G; G.hasev = 0; G.fk = 0; G.lk = 0; G.closed = 0; G.tn = 0; G.tail = 0;     // tiles nearer than the window
+    Agg G; G.hasev = 0; G.fk = 0; G.lk = 0; G.closed = 0; G.tn = 0; G.tail = 0;     // items nearer than the window
     Pre X; X.T = 0; X.o.q = 0; X.o.r = 0; X.cnt = 0; X.tail = 0;
-    for (int base = tile - 1; base >= 0; base -= 32) {
+    ready = true;
+    const int p = tile & 31, grp = tile >> 5;
+    Win w;
+    // ---- level 0: the predecessors inside the tile's own group (lane l <-> tile - 1 - l, l < p) ------------------
+    if (p > 0) {
+        w.a0 = w.a1 = w.i0 = w.i1 = make_uint4(0, 0, 0, 0);
+        w.st = ST_AGG;                                   // lanes >= p: not part of this window
+        if (lane < p) {
+            const TileDesc &Dj = A.descs[tile - 1 - lane];
+            w.i0 = ld_vol128(&Dj.i0); w.i1 = ld_vol128(&Dj.i1); w.a0 = ld_vol128(&Dj.a0); w.a1 = ld_vol128(&Dj.a1);
+            w.st = (w.i0.x == tagI && w.i1.x == tagI) ? ST_INCL : ((w.a0.x == tagA && w.a1.x == tagA) ? ST_AGG : ST_EMPTY);
+        }
+        const uint32_t ib = __ballot_sync(FULL, w.st == ST_INCL);
+        const int f = ib ? __ffs(ib) - 1 : p;            // nearest tile with an inclusive prefix
+        const uint32_t empty = __ballot_sync(FULL, w.st == ST_EMPTY);
+        if (p == 31) {
+            // last tile of its group: the group aggregate goes out as soon as all 32 tile aggregates are there
+            const uint32_t noagg = __ballot_sync(FULL, lane < 31 && !(w.a0.x == tagA && w.a1.x == tagA));
+            if (noagg) { ready = force; return X; }
+            const Agg Wall = fold_window(w, 31, P, lane);
+            const Agg GG = agg_combine(Wall, own, P);
+            if (lane == 0) publish_agg(&A.gdescs[grp], tagA, GG);
+        }
+        if (empty & ((1u << f) - 1u)) { ready = force; return X; }      // (forced: the chain is broken, the status word says so)
+        const Agg W = fold_window(w, f, P, lane);
+        if (ib) return pre_extend(incl_at(w, f), W, P);
+        G = W;
+    }
+    // ---- level 1: whole groups (lane l <-> group base - l): group aggregate, or the inclusive prefix of its last tile
+    for (int base = grp - 1; base >= 0; base -= 32) {
         const int j = base - lane;
-        uint4 wa = make_uint4(0, 0, 0, 0), wb = wa, w0 = wa, w1 = wa;
-        uint32_t st = ST_INCL;                           // tiles before 0 carry the empty inclusive prefix
-        int f = 32; bool ok = true;
-        for (int spins = 0;; ++spins) {
-            if (j >= 0) {
-                const TileDesc &Dj = A.descs[j];
-                w0 = ld_vol128(&Dj.i0); w1 = ld_vol128(&Dj.i1); wa = ld_vol128(&Dj.a0); wb = ld_vol128(&Dj.a1);
-                st = (w0.x == tagI && w1.x == tagI) ? ST_INCL : ((wa.x == tagA && wb.x == tagA) ? ST_AGG : ST_EMPTY);
-            }
-            const uint32_t ib = __ballot_sync(FULL, st == ST_INCL);
-            f = ib ? __ffs(ib) - 1 : 32;                 // nearest tile with an inclusive prefix
-            const uint32_t missing = __ballot_sync(FULL, st == ST_EMPTY) & (f < 32 ? ((1u << f) - 1u) : FULL);
-            if (!missing) break;
-            if (spins > SPIN_LIMIT) { ok = false; break; }
-            __nanosleep(40);
+        w.a0 = w.a1 = w.i0 = w.i1 = make_uint4(0, 0, 0, 0);
+        w.st = ST_INCL;                                  // groups before 0 carry the empty inclusive prefix
+        if (j >= 0) {
+            const TileDesc &Dt = A.descs[32 * j + 31];
+            const TileDesc &Dg = A.gdescs[j];
+            w.i0 = ld_vol128(&Dt.i0); w.i1 = ld_vol128(&Dt.i1); w.a0 = ld_vol128(&Dg.a0); w.a1 = ld_vol128(&Dg.a1);
+            w.st = (w.i0.x == tagI && w.i1.x == tagI) ? ST_INCL : ((w.a0.x == tagA && w.a1.x == tagA) ? ST_AGG : ST_EMPTY);
         }
-        if (!ok) { if (lane == 0) A.status[1] = 1u; return X; }
-        // lanes < f hold aggregates (far = high lane)
-        const bool in = lane < f;
-        const int fk_l = in ? (int)wa.y : 0, lk_l = (int)wa.z, cl_l = (int)(wa.w & 0x7fffffffu);
-        const bool ev_l = in && (wa.w >> 31);
-        int Ps = fk_l;                                   // kept-before-first-start summed over lanes >= this one
-#pragma unroll
-        for (int d = 1; d < 32; d <<= 1) { const int t = __shfl_down_sync(FULL, Ps, d); if (lane + d < 32) Ps += t; }
-        const uint32_t evmask = __ballot_sync(FULL, ev_l);
-        const int P0 = __shfl_sync(FULL, Ps, 0);
-        // the window's lanes < f as one aggregate W
-        Agg W; W.hasev = evmask != 0; W.closed = 0;
-        if (!evmask) { W.fk = P0; W.lk = P0; }
-        else {
-            const uint32_t higher = lane == 31 ? 0u : (evmask & ~((2u << lane) - 1u));
-            const int ep = higher ? __ffs(higher) - 1 : -1;          // next farther tile with a record start
-            const int P_ep = __shfl_sync(FULL, Ps, ep < 0 ? 0 : ep), lk_ep = __shfl_sync(FULL, lk_l, ep < 0 ? 0 : ep);
-            int t32 = 0;
-            if (ev_l) t32 = cl_l + (ep >= 0 ? tok_count32(lk_ep + Ps - P_ep, P) : 0);
-            W.closed = __reduce_add_sync(FULL, t32);
-            const int e1 = 31 - __clz(evmask), e0 = __ffs(evmask) - 1;
-            W.fk = __shfl_sync(FULL, Ps, e1);
-            W.lk = __shfl_sync(FULL, lk_l, e0) + P0 - __shfl_sync(FULL, Ps, e0);
-        }
-        W.tn = 0; W.tail = 0;
-        if (P.mode == MODE_KMER && k > 1) {
-            const unsigned long long mytail = (unsigned long long)wb.z | ((unsigned long long)((wb.y >> 4) & 0x3ffu) << 32);
-            const int mycnt = (int)(wb.y & 15u);
-            const int want = min(k - 1, W.lk);
-            for (int l = 0; l < f && W.tn < want; ++l) {
-                const unsigned long long tl = __shfl_sync(FULL, mytail, l);
-                const int cn = min(__shfl_sync(FULL, mycnt, l), want - W.tn);
-                W.tail |= low_classes(tl, cn) << (3 * W.tn);
-                W.tn += cn;
-                if ((evmask >> l) & 1u) break;
-            }
-        }
+        const uint32_t ib = __ballot_sync(FULL, w.st == ST_INCL);
+        const int f = ib ? __ffs(ib) - 1 : 32;
+        const uint32_t missing = __ballot_sync(FULL, w.st == ST_EMPTY) & (f < 32 ? ((1u << f) - 1u) : FULL);
+        if (missing) { ready = force; return X; }
+        const Agg W = fold_window(w, f, P, lane);
         if (f < 32) {
-            // the inclusive prefix at lane f (tiles before 0: empty), extended by W, then by the nearer tiles G
-            Pre F;
-            const int64_t fT = (int64_t)(((uint64_t)w0.z << 32) | w0.y), fq = (int64_t)(((uint64_t)w1.z << 32) | w1.y);
-            const unsigned long long ftail = (unsigned long long)w1.w | ((unsigned long long)((w0.w >> 8) & 0x3ffu) << 32);
-            F.T = __shfl_sync(FULL, fT, f); F.o.q = __shfl_sync(FULL, fq, f);
-            const uint32_t fw = __shfl_sync(FULL, w0.w, f);
-            F.o.r = (int32_t)(fw & 15u); F.cnt = (int)((fw >> 4) & 15u);
-            F.tail = __shfl_sync(FULL, ftail, f);
+            Pre F = incl_at(w, f);
+            if (base - f < 0) { F = X; }                 // walked past group 0: the empty prefix
             return pre_extend(pre_extend(F, W, P), G, P);
         }
         G = agg_combine(W, G, P);

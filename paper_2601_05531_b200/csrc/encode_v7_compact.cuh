@@ -5,8 +5,8 @@
 namespace dtk {
 
 // byte q (0..63) of this lane's staged 64 bytes
-__device__ __forceinline__ uint32_t staged_byte(const uint4 *slot, int sw, int q) {
-    return reinterpret_cast<const uint8_t *>(slot)[(((q >> 4) ^ sw) << 4) | (q & 15)];
+__device__ __forceinline__ uint32_t staged_byte(const uint4 *slot, int q) {
+    return reinterpret_cast<const uint8_t *>(slot)[q];
 }
 
 // ---- entry line state of a region, read off the 128 bytes in front of it when they settle it ---------------------
@@ -187,17 +187,21 @@ __device__ __forceinline__ void append_step(uint32_t *cst, uint32_t *fst, const 
     if (__all_sync(FULL, n >= 32)) {
         if (!(lane & 1)) {
             if (lane == 0) { if (csh) cw[0] |= cp[0]; if (fsh) fw[0] |= fp[0]; }
+            cp[0] = cw[0]; cp[1] = cw[1];                        // n >= 32: at least 64 code bits and 32 flag bits
 #pragma unroll
-            for (int i = 0; i < 5; ++i) if (32 * i < cend) cp[i] = cw[i];
+            for (int i = 2; i < 5; ++i) if (32 * i < cend) cp[i] = cw[i];
+            fp[0] = fw[0];
 #pragma unroll
-            for (int i = 0; i < 3; ++i) if (32 * i < fend) fp[i] = fw[i];
+            for (int i = 1; i < 3; ++i) if (32 * i < fend) fp[i] = fw[i];
         }
         __syncwarp();
         if (lane & 1) {
+            cp[0] |= cw[0]; cp[1] |= cw[1];
 #pragma unroll
-            for (int i = 0; i < 5; ++i) if (32 * i < cend) cp[i] |= cw[i];
+            for (int i = 2; i < 5; ++i) if (32 * i < cend) cp[i] |= cw[i];
+            fp[0] |= fw[0];
 #pragma unroll
-            for (int i = 0; i < 3; ++i) if (32 * i < fend) fp[i] |= fw[i];
+            for (int i = 1; i < 3; ++i) if (32 * i < fend) fp[i] |= fw[i];
         }
         __syncwarp();
     } else {
@@ -212,11 +216,13 @@ __device__ __forceinline__ void append_step(uint32_t *cst, uint32_t *fst, const 
 }
 
 // ---- one region ---------------------------------------------------------------------------------------------------
-// ent_ls: entry line state to use when `given` (second pass over a tile), else it is read off the bytes in front of
-// the region or assumed IN_LINE.
+// The entry line state is read off the bytes in front of the region, or assumed IN_LINE when they do not settle it.
+// The assumption can only be wrong inside a header line longer than that window; all it then costs is that the kept
+// bases in front of the region's first line reset (hfix of them) must be dropped, which the scan warp does by moving
+// the region's first slot -- no second pass.
 template <bool DENSE>
 __device__ __forceinline__ void compact_region(const EncArgs &A, Smem7 &sm, TileBuf &tb, uint32_t *st, int tile, int warp, int lane,
-                                               bool given, uint32_t ent_ls, int64_t pos_first, int64_t pos_last) {
+                                               int64_t pos_first, int64_t pos_last) {
     constexpr uint32_t FULL = 0xffffffffu;
     const EncParams &P = A.prm;
     const int S = A.S;
@@ -241,12 +247,10 @@ __device__ __forceinline__ void compact_region(const EncArgs &A, Smem7 &sm, Tile
     }
     // line state carried along the region (warp-uniform) and the region's summary as a function of its entry state
     uint32_t ls = LS_IN_LINE, known = 1, r_hr = 0, r_x = LS_LINE_START;
+    int hfix = -1;                                               // -1: no line reset seen yet
     if (!DENSE && P.strip_headers) {
-        if (given) ls = ent_ls;
-        else {
-            ls = region_entry_state(A, sm, tb, t0, rs0, lane, pos_first, pos_last);
-            if (ls == LS_UNKNOWN) { known = 0; ls = LS_IN_LINE; }
-        }
+        ls = region_entry_state(A, sm, tb, t0, rs0, lane, pos_first, pos_last);
+        if (ls == LS_UNKNOWN) { known = 0; ls = LS_IN_LINE; }
     }
     const uint32_t ls_entry = ls;
     // record starts inside the region: events [ev, re_hi) of the tile's list (m <= EV_MAX)
@@ -262,22 +266,25 @@ __device__ __forceinline__ void compact_region(const EncArgs &A, Smem7 &sm, Tile
     }
     __syncwarp();
     int cnt = 0;                                                 // kept bases of the region so far
-    const uint4 *slot = &sm.stage[warp][lane * 4];
-    const int sw = (lane >> 1) & 3;
+    uint4 *const slot = &sm.stage[warp][lane * 4];
+    // everything inside the loop is region-relative and 32 bits wide (clamped where the 64-bit value is out of range)
+    auto rel32 = [&](int64_t pos) -> int { const int64_t dlt = pos - rs0; return dlt < -(1 << 30) ? -(1 << 30) : (dlt > (1 << 30) ? (1 << 30) : (int)dlt); };
+    const int end_rel = rel32(A.p_end), first_rel = rel32(pos_first), last_rel = rel32(pos_last);
+    const uint4 *const src_lane = reinterpret_cast<const uint4 *>(A.bytes_al + rs0) + lane * 4;
 #pragma unroll 1
     for (int s = 0; s < S; ++s) {
-        const int64_t ws0 = rs0 + (int64_t)s * WB;               // position of the warp's first byte
-        const int64_t p0 = ws0 + (int64_t)lane * LB;
-        if (ws0 > A.p_end) break;                                // (warp-uniform) nothing left; position p_end itself may hold the closing record offset
+        const int w0r = s * WB;                                  // region offset of the warp's first byte
+        const int p0r = w0r + lane * LB;                         //   and of this lane's
+        if (w0r > end_rel) break;                                // (warp-uniform) nothing left; position p_end itself may hold the closing record offset
         uint4 v[4];
         {
-            const uint4 *src = reinterpret_cast<const uint4 *>(A.bytes_al + p0);
-            if (ws0 + WB <= A.p_end) {
+            const uint4 *src = src_lane + s * (WB / 16);
+            if (w0r + WB <= end_rel) {
 #pragma unroll
                 for (int j = 0; j < 4; ++j) v[j] = __ldg(src + j);
             } else {
 #pragma unroll
-                for (int j = 0; j < 4; ++j) v[j] = (p0 + 16 * j < A.p_end) ? __ldg(src + j) : make_uint4(0, 0, 0, 0);
+                for (int j = 0; j < 4; ++j) v[j] = (p0r + 16 * j < end_rel) ? __ldg(src + j) : make_uint4(0, 0, 0, 0);
             }
         }
         uint32_t C[4];
@@ -291,15 +298,14 @@ __device__ __forceinline__ void compact_region(const EncArgs &A, Smem7 &sm, Tile
         // which bytes need their digit / flag corrected if they are kept
         unsigned long long skip = 0, nl = 0, gt = 0, fix = 0;
         if (E) {
-            uint4 *wslot = &sm.stage[warp][lane * 4];
 #pragma unroll
-            for (int j = 0; j < 4; ++j) wslot[j ^ sw] = v[j];
+            for (int j = 0; j < 4; ++j) slot[j] = v[j];         // (bank conflicts cost LSU cycles, which are plentiful; a swizzle costs ALU)
             unsigned long long rem = E;
             while (rem) {
                 const int q = __clzll((long long)rem);
                 const unsigned long long bq = bit_at(q);
                 rem ^= bq;
-                const uint32_t byte = staged_byte(slot, sw, q);
+                const uint32_t byte = staged_byte(slot, q);
                 const uint32_t c = sm.lut[byte];
                 if (byte == '\n') nl |= bq;
                 if (byte == '>') gt |= bq;
@@ -315,7 +321,7 @@ __device__ __forceinline__ void compact_region(const EncArgs &A, Smem7 &sm, Tile
                 const int q = __clzll((long long)rem);
                 const unsigned long long bq = bit_at(q);
                 rem ^= bq;
-                const uint32_t c = sm.lut[staged_byte(slot, sw, q)];
+                const uint32_t c = sm.lut[staged_byte(slot, q)];
                 if (c < CLS_N) bad &= ~bq;
                 set_digit(C, q, c < CLS_N ? c : (c == CLS_N ? 2u : 1u));
             }
@@ -347,12 +353,13 @@ __device__ __forceinline__ void compact_region(const EncArgs &A, Smem7 &sm, Tile
                     rs = sm.wk[warp][lane];
                 }
             } else {
-                e_cnt = warp_events_many(A, sm.wk[warp], r_lo, m, ws0, lane, e_lo);
+                e_cnt = warp_events_many(A, sm.wk[warp], r_lo, m, rs0 + w0r, lane, e_lo);
                 if (e_cnt) { __syncwarp(); rs = sm.wk[warp][lane]; }
             }
         }
         // ---- line state and header mask -----------------------------------------------------------------------------
         unsigned long long hdr = 0;
+        bool first_reset = false;                                // (warp-uniform) the region's first line reset is in this step
         if (P.strip_headers) {
             const unsigned long long osk = skip & ~nl & ~gt;     // SKIP bytes that neither end nor start a line
             uint32_t c_hr, c_x;
@@ -371,13 +378,14 @@ __device__ __forceinline__ void compact_region(const EncArgs &A, Smem7 &sm, Tile
                 hdr = R.hdr; c_hr = R.c_hr; c_x = R.c_x;
             }
             ls = ls_apply(c_hr, c_x, ls);
+            first_reset = !known && hfix < 0 && c_hr;
             r_x = ls_apply(c_hr, c_x, r_x); r_hr |= c_hr;
         }
         unsigned long long keep = ~skip & ~hdr;
-        if (p0 < pos_first || p0 + LB > pos_last) {
-            const int64_t ia = pos_first - p0, ib = pos_last - p0;       // in-record positions are [ia, ib)
-            const unsigned long long ma = ia <= 0 ? ~0ull : from_pos((int)(ia > 64 ? 64 : ia));
-            const unsigned long long mb = ib <= 0 ? 0ull : (ib >= 64 ? ~0ull : ~from_pos((int)ib));
+        if (p0r < first_rel || p0r + LB > last_rel) {
+            const int ia = first_rel - p0r, ib = last_rel - p0r;         // in-record positions are [ia, ib)
+            const unsigned long long ma = ia <= 0 ? ~0ull : from_pos(ia > 64 ? 64 : ia);
+            const unsigned long long mb = ib <= 0 ? 0ull : (ib >= 64 ? ~0ull : ~from_pos(ib));
             keep &= ma & mb;
         }
         {
@@ -387,7 +395,7 @@ __device__ __forceinline__ void compact_region(const EncArgs &A, Smem7 &sm, Tile
                 const int q = __clzll((long long)rem);
                 const unsigned long long bq = bit_at(q);
                 rem ^= bq;
-                const uint32_t c = sm.lut[staged_byte(slot, sw, q)];
+                const uint32_t c = sm.lut[staged_byte(slot, q)];
                 if (c < CLS_N) bad &= ~bq;
                 set_digit(C, q, c < CLS_N ? c : (c == CLS_N ? 2u : 1u));
             }
@@ -410,6 +418,13 @@ __device__ __forceinline__ void compact_region(const EncArgs &A, Smem7 &sm, Tile
             total = __shfl_sync(FULL, inc, 31);
         }
         append_step(cst, fst, C, bad, cnt + a, n, lane);
+        if (first_reset) {
+            // kept bases (under the IN_LINE assumption) in front of the first '\n' or record start of the region
+            const unsigned long long rz = nl | rs;
+            const int L = __ffs(__ballot_sync(FULL, rz != 0ull)) - 1;
+            const int q = first_pos(rz);
+            hfix = cnt + __shfl_sync(FULL, a + (q ? __popcll(keep >> (64 - q)) : 0), L);
+        }
         if (e_cnt) {                                             // (warp-uniform) kept bases in front of each record start
             sm.wk[warp][lane] = keep; sm.offw[warp][lane] = (uint16_t)a;
             __syncwarp();
@@ -425,6 +440,7 @@ __device__ __forceinline__ void compact_region(const EncArgs &A, Smem7 &sm, Tile
     }
     if (lane == 0) {
         tb.reg_cnt[warp] = DENSE ? RB : cnt;
+        tb.reg_hfix[warp] = hfix < 0 ? cnt : hfix;
         tb.reg_ls[warp] = (known << 8) | (ls_entry << 4) | (r_hr << 2) | r_x;
     }
 }

@@ -3,9 +3,19 @@
 
 namespace dtk {
 
+#ifdef DTK_PROF
+#define PROF_T(var) const long long var = clock64()
+#define PROF_ADD(slot, t0, t1) do { if (lane == 0) atomicAdd(&A.prof[slot], (unsigned long long)((t1) - (t0))); } while (0)
+#define PROF_INC(slot) do { if (lane == 0) atomicAdd(&A.prof[slot], 1ull); } while (0)
+#else
+#define PROF_T(var)
+#define PROF_ADD(slot, t0, t1)
+#define PROF_INC(slot)
+#endif
+
 // KK: the emission variant compiled in -- 0 single-nt, 1..6 / 8 that k, -1 every variant behind a run-time switch.
 // Loop iteration i of a CTA:   compute warps: compact tile B_i -> DONE -> (READY) emit tile B_{i-1}
-//                              scan warp:     prefix + tables of B_{i-1} -> READY; (DONE) aggregate of B_i; prepare B_{i+1} -> PREP
+//                              scan warp:     prefix + tables of B_{i-1} -> READY || (DONE) aggregate of B_i; then prepare B_{i+1} -> PREP
 template <typename IdT, int KK, bool DENSE>
 __global__ void __launch_bounds__(NT7, 3) encode_tiles_v7(const __grid_constant__ EncArgs A) {
     extern __shared__ __align__(16) uint8_t smem_raw[];
@@ -16,66 +26,88 @@ __global__ void __launch_bounds__(NT7, 3) encode_tiles_v7(const __grid_constant_
     const int64_t pos_first = rec_pos(A, 0), pos_last = rec_pos(A, A.n_rec);   // bytes outside are in no record
 
     if (tid < 256) sm.lut[tid] = A.lut[tid];
+    if (tid == 0) sm.done_cnt = 0;
     __syncthreads();
 
     if (warp == NWC) {
         // =============================================== scan warp ===================================================
+        // Iteration i of the compute warps compacts tile B_i and then emits B_{i-1}; the scan warp runs one message
+        // ahead: PREP(i+1) goes out at the start of iteration i, so the compute warps never wait for a sibling warp or
+        // for this warp between tiles -- only READY(i) needs every region of B_{i-1} (finished a whole tile ago).
         unsigned long long ticket = 0;
         if (lane == 0) ticket = atomicAdd(A.ticket, 1ull);
         ticket = __shfl_sync(FULL, ticket, 0);
         int bufB = 0;
-        int tileB = scan_prep(A, sm.tb[bufB], ticket, lane);
+        int tileB = scan_prep(A, sm.tb[0], ticket, lane);
         if (lane == 0) {
             TileCtl &c = sm.ctl[0];
-            c.tile = tileB; c.buf = bufB; c.emit = 0; c.emit_buf = 0; c.emit_generic = 0; c.redo = 0; c.last = tileB < 0;
+            c.tile = tileB; c.buf = 0; c.emit = 0; c.emit_buf = 0; c.emit_generic = 0; c.last = tileB < 0;
         }
         __threadfence_block();
         bar_arrive(BAR_PREP);
-        if (tileB >= 0) {
+        bool pendA = false;                                // the tile in bufB ^ 1 still waits for its prefix + tables
+        bool force = false;
+        int done_target = 0, spins = 0, it = 0;
+        auto stuck = [&]() {                               // bounded wait: a broken chain sets the status word instead of hanging
+            if (++spins > SPIN_LIMIT / 4) { if (lane == 0) A.status[1] = 1u; force = true; }
+            __nanosleep(64);
+        };
+#pragma unroll 1
+        for (; tileB >= 0; ++it) {
+            TileBuf &tbB = sm.tb[bufB];
+            if (pendA && scan_tables<DENSE>(A, sm, sm.tb[bufB ^ 1], sm.strm[bufB ^ 1], lane, force)) {
+                __threadfence_block();
+                bar_arrive(BAR_READY + (it & 1));
+                pendA = false;
+            }
+            // ---- next tile into the other buffer (the preparation only touches tile / m / rlo / ev_p, which neither
+            //      the tables nor the emission of the tile held there read any more)
+            PROF_T(p0);
             if (lane == 0) ticket = atomicAdd(A.ticket, 1ull);
             ticket = __shfl_sync(FULL, ticket, 0);
-        }
-        bool emitA = false;                                // this iteration ends with the emission of the tile in bufB ^ 1
-        int rdy = 0;                                       // READY alternates between two barrier ids
-#pragma unroll 1
-        for (int it = 0; tileB >= 0 || emitA; ++it) {
-            TileCtl &nx = sm.ctl[(it + 1) & 1];
-            if (emitA) {
-                TileBuf &ta = sm.tb[bufB ^ 1];
-                scan_tables<DENSE>(A, sm, ta, sm.strm[bufB ^ 1], lane);
-                __threadfence_block();
-                bar_arrive(BAR_READY + rdy);
-                rdy ^= 1;
-            }
-            if (tileB < 0) break;                          // that was the last emission
-            bar_sync(BAR_DONE);
-            TileBuf &tbB = sm.tb[bufB];
-            uint32_t ent[NWC];
-            if (scan_regions<DENSE>(A, tbB, lane, ent)) {
-                // some region assumed a wrong entry line state: the compute warps go over the tile again
-                if (lane == 0) {
-                    nx.tile = tileB; nx.buf = bufB; nx.emit = 0; nx.emit_buf = 0; nx.emit_generic = 0; nx.redo = 1; nx.last = 0;
-#pragma unroll
-                    for (int w = 0; w < NWC; ++w) nx.ent_ls[w] = ent[w];
-                }
-                __threadfence_block();
-                bar_arrive(BAR_PREP);
-                emitA = false;
-                continue;
-            }
-            scan_aggregate<DENSE>(A, tbB, sm.strm[bufB], lane);
-            // next tile into the other buffer
-            const int tileC = scan_prep(A, sm.tb[bufB ^ 1], ticket, lane);   // (its tables were last read two iterations ago)
+            const int tileC = scan_prep(A, sm.tb[bufB ^ 1], ticket, lane);
+            PROF_T(p1); PROF_ADD(0, p0, p1);
             if (lane == 0) {
-                nx.tile = tileC; nx.buf = bufB ^ 1; nx.emit = 1; nx.emit_buf = bufB; nx.emit_generic = tbB.m > EV_MAX; nx.redo = 0; nx.last = tileC < 0;
+                TileCtl &nx = sm.ctl[(it + 1) & 1];
+                nx.tile = tileC; nx.buf = bufB ^ 1; nx.emit = 1; nx.emit_buf = bufB; nx.emit_generic = tbB.m > EV_MAX; nx.last = tileC < 0;
             }
             __threadfence_block();
-            bar_arrive(BAR_PREP);
-            if (tileC >= 0) {
-                if (lane == 0) ticket = atomicAdd(A.ticket, 1ull);
-                ticket = __shfl_sync(FULL, ticket, 0);
+            bar_arrive(BAR_PREP + ((it + 1) & 1));
+            // ---- two jobs, neither of which may hold up the other: prefix + tables of the tile to emit (needs the
+            //      predecessors' aggregates), aggregate of the tile being compacted (needs the compute warps)
+            PROF_T(p2);
+            for (bool needD = true; pendA || needD;) {
+                bool progress = false;
+                if (pendA && scan_tables<DENSE>(A, sm, sm.tb[bufB ^ 1], sm.strm[bufB ^ 1], lane, force)) {
+                    __threadfence_block();
+                    bar_arrive(BAR_READY + (it & 1));
+                    pendA = false; progress = true;
+                }
+                if (needD && *(volatile int32_t *)&sm.done_cnt >= done_target + NWC) {
+                    __threadfence_block();
+                    done_target += NWC;
+                    PROF_T(a0);
+                    scan_regions<DENSE>(A, tbB, lane);
+                    scan_aggregate<DENSE>(A, tbB, sm.strm[bufB], lane);
+                    PROF_T(a1); PROF_ADD(2, a0, a1);
+                    needD = false; progress = true;
+                }
+                if (!progress) stuck(); else spins = 0;
             }
-            tileB = tileC; bufB ^= 1; emitA = true;
+            // ---- the tile just aggregated gets its prefix right away: the sooner its inclusive prefix is out, the
+            //      shorter every successor's walk back (its emission is a whole tile away)
+            PROF_T(p3); PROF_ADD(1, p2, p3);
+            if (scan_tables<DENSE>(A, sm, tbB, sm.strm[bufB], lane, force)) {
+                __threadfence_block();
+                bar_arrive(BAR_READY + ((it + 1) & 1));
+            } else { pendA = true; PROF_INC(4); }
+            PROF_T(p4); PROF_ADD(3, p3, p4); PROF_INC(5);
+            tileB = tileC; bufB ^= 1;
+        }
+        if (pendA) {
+            while (!scan_tables<DENSE>(A, sm, sm.tb[bufB ^ 1], sm.strm[bufB ^ 1], lane, force)) stuck();
+            __threadfence_block();
+            bar_arrive(BAR_READY + (it & 1));
         }
         return;
     }
@@ -84,23 +116,26 @@ __global__ void __launch_bounds__(NT7, 3) encode_tiles_v7(const __grid_constant_
     const bool affine = P.nt_ids[1] == P.nt_ids[0] + 1 && P.nt_ids[2] == P.nt_ids[0] + 2 && P.nt_ids[3] == P.nt_ids[0] + 3;
     const bool vec_ok = (reinterpret_cast<uintptr_t>(A.ids) & 15) == 0 &&
                         (P.mode != MODE_KMER || (P.k >= 1 && P.k <= 6) || P.k == 8);
-    int rdy = 0;
 #pragma unroll 1
     for (int it = 0;; ++it) {
-        bar_sync(BAR_PREP);
+        PROF_T(c0);
+        bar_sync(BAR_PREP + (it & 1));
+        PROF_T(c1); if (warp == 0) PROF_ADD(8, c0, c1);
         const TileCtl &c = sm.ctl[it & 1];
         const int tile = c.tile, buf = c.buf, emit = c.emit, ebuf = c.emit_buf, egen = c.emit_generic, last = c.last;
         if (tile >= 0) {
-            compact_region<DENSE>(A, sm, sm.tb[buf], sm.strm[buf], tile, warp, lane, c.redo != 0, c.ent_ls[warp], pos_first, pos_last);
-            __threadfence_block();
-            bar_arrive(BAR_DONE);
+            compact_region<DENSE>(A, sm, sm.tb[buf], sm.strm[buf], tile, warp, lane, pos_first, pos_last);
+            __syncwarp();
+            if (lane == 0) { __threadfence_block(); atomicAdd(&sm.done_cnt, 1); }
         }
+        PROF_T(c2); if (warp == 0) PROF_ADD(9, c1, c2);
         if (emit) {
-            bar_sync(BAR_READY + rdy);
-            rdy ^= 1;
+            bar_sync(BAR_READY + (it & 1));
+            PROF_T(c3); if (warp == 0) PROF_ADD(10, c2, c3);
             const TileBuf &ta = sm.tb[ebuf];
             if (egen) emit_generic<IdT, DENSE>(A, sm.strm[ebuf], ta, tid);
             else emit_region<IdT, KK>(A, sm.strm[ebuf], ta, warp, lane, vec_ok, affine);
+            PROF_T(c4); if (warp == 0) PROF_ADD(11, c3, c4);
         }
         if (last) break;
     }

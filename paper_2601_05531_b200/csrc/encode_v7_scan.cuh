@@ -55,10 +55,11 @@ __device__ __noinline__ uint32_t ls_chain_state(const EncArgs &A, int tile, int 
     return have_carry ? carry : LS_LINE_START;
 }
 
-// ---- after the compute warps finished a tile: region prefix, line-state check --------------------------------------
-// Returns true when some region ran under a wrong entry-state assumption; the exact entry states are then in ent[].
+// ---- after the compute warps finished a tile: line-state check, region prefix ---------------------------------------
+// A region that assumed IN_LINE but really started inside a header line loses the kept bases in front of its first
+// line reset: its first slot moves up by that many (rbase) and its count shrinks.
 template <bool DENSE>
-__device__ __forceinline__ bool scan_regions(const EncArgs &A, TileBuf &tb, int lane, uint32_t *ent) {
+__device__ __forceinline__ void scan_regions(const EncArgs &A, TileBuf &tb, int lane) {
     constexpr uint32_t FULL = 0xffffffffu;
     const EncParams &P = A.prm;
     const int tile = tb.tile;
@@ -66,19 +67,15 @@ __device__ __forceinline__ bool scan_regions(const EncArgs &A, TileBuf &tb, int 
     if (DENSE) {
         const int RB = A.S * WB;
         if (lane <= NWC) tb.cum[lane] = lane * RB;
+        if (lane < NWC) tb.rbase[lane] = reg_slot(lane);
         if (lane == 0) {
             const int64_t rem = rec_pos(A, A.n_rec) - t0;
             tb.ktot = rem < 0 ? 0 : (rem > TBS ? (int)TBS : (int)rem);
         }
         __syncwarp();
-        return false;
+        return;
     }
-    int c = lane < NWC ? tb.reg_cnt[lane] : 0, inc = c;
-#pragma unroll
-    for (int d = 1; d < NWC; d <<= 1) { const int t = __shfl_up_sync(FULL, inc, d); if (lane >= d) inc += t; }
-    if (lane < NWC) tb.cum[lane] = inc - c;
-    if (lane == NWC - 1) { tb.cum[NWC] = inc; tb.ktot = inc; }
-    bool redo = false;
+    uint32_t dropmask = 0;                                 // regions that started inside a header line unawares
     if (P.strip_headers) {
         const uint32_t tagL = A.gen << 8;
         uint32_t rl[NWC];
@@ -96,13 +93,17 @@ __device__ __forceinline__ bool scan_regions(const EncArgs &A, TileBuf &tb, int 
         if (lane == 0) st_vol32(&A.ls[tile], tagL | (LK_FINAL << 2) | ls_apply(t_hr, t_x, state));
 #pragma unroll
         for (int w = 0; w < NWC; ++w) {
-            ent[w] = state;
-            if (!((rl[w] >> 8) & 1u) && state != LS_IN_LINE) redo = true;
+            if (!((rl[w] >> 8) & 1u) && state == LS_IN_HEADER) dropmask |= 1u << w;
             state = ls_apply((rl[w] >> 2) & 1u, rl[w] & 3u, state);
         }
     }
+    const int drop = (lane < NWC && ((dropmask >> lane) & 1u)) ? tb.reg_hfix[lane] : 0;
+    int c = lane < NWC ? tb.reg_cnt[lane] - drop : 0, inc = c;
+#pragma unroll
+    for (int d = 1; d < NWC; d <<= 1) { const int t = __shfl_up_sync(FULL, inc, d); if (lane >= d) inc += t; }
+    if (lane < NWC) { tb.cum[lane] = inc - c; tb.rbase[lane] = reg_slot(lane) + drop; }
+    if (lane == NWC - 1) { tb.cum[NWC] = inc; tb.ktot = inc; }
     __syncwarp();
-    return redo;
 }
 
 // logical kept-base index in front of record start e of the tile
@@ -123,9 +124,15 @@ __device__ __forceinline__ void scan_aggregate(const EncArgs &A, TileBuf &tb, co
     if (!DENSE) {
         // region-relative -> logical
         if (m <= EV_MAX) {
-            for (int e = lane; e < m; e += 32) { const int v = tb.ev_k[e]; tb.ev_k[e] = (v & 0xffff) + tb.cum[v >> 16]; }
+            for (int e = lane; e < m; e += 32) {
+                const int v = tb.ev_k[e], w = v >> 16;
+                tb.ev_k[e] = max((v & 0xffff) - (tb.rbase[w] - reg_slot(w)), 0) + tb.cum[w];
+            }
         } else {
-            for (int e = lane; e < m; e += 32) { const int v = __ldcg(A.rec_k + tb.rlo + e); A.rec_k[tb.rlo + e] = (v & 0xffff) + tb.cum[v >> 16]; }
+            for (int e = lane; e < m; e += 32) {
+                const int v = __ldcg(A.rec_k + tb.rlo + e), w = v >> 16;
+                A.rec_k[tb.rlo + e] = max((v & 0xffff) - (tb.rbase[w] - reg_slot(w)), 0) + tb.cum[w];
+            }
         }
         __syncwarp();
     }
@@ -171,23 +178,38 @@ __device__ __forceinline__ void scan_aggregate(const EncArgs &A, TileBuf &tb, co
         TileAgg &g = tb.ag;
         g.fk = fk; g.lk = lk; g.closed = closed; g.tn = tn; g.hasev = m > 0; g.tail = gtail;
         tb.ntok = ntok_ev;
+        tb.e_tile = tile; tb.e_m = m; tb.e_rlo = tb.rlo;   // (tile / m / rlo / ev_p belong to the next tile's preparation from here on)
     }
     __syncwarp();
 }
 
+// class c (0..5) into stream slot u, whatever the slot held (single lanes of the scan warp; other lanes may hit the same word)
+__device__ __forceinline__ void put_class(uint32_t *st, int u, uint32_t c) {
+    const uint32_t dg = c < CLS_N ? c : (c == CLS_N ? 2u : 1u);
+    const int sh = 30 - 2 * (u & 15);
+    atomicAnd(&st[u >> 4], ~(3u << sh));
+    atomicOr(&st[u >> 4], dg << sh);
+    const uint32_t fb = 1u << (31 - (u & 31));
+    if (c >= CLS_N) atomicOr(&st[SW_CODE + (u >> 5)], fb); else atomicAnd(&st[SW_CODE + (u >> 5)], ~fb);
+}
+
 // ---- prefix of a tile, its segment table, out_offsets, halo -------------------------------------------------------
+// Returns false (nothing changed) when a predecessor the look-back needs has not published yet.
 template <bool DENSE>
-__device__ __forceinline__ void scan_tables(const EncArgs &A, const Smem7 &sm, TileBuf &tb, uint32_t *st, int lane) {
+__device__ __forceinline__ bool scan_tables(const EncArgs &A, const Smem7 &sm, TileBuf &tb, uint32_t *st, int lane, bool force) {
     constexpr uint32_t FULL = 0xffffffffu;
     const EncParams &P = A.prm;
-    const int k = P.k, m = tb.m, tile = tb.tile, ktot = tb.ktot;
-    const int64_t t0 = (int64_t)tile * A.S * TB;
+    const int k = P.k, m = tb.e_m, tile = tb.e_tile, ktot = tb.ktot;
+    const int64_t t0 = (int64_t)tile * A.S * TB, rlo = tb.e_rlo;
+    auto kept = [&](int e) -> int { return DENSE ? (int)(rec_pos(A, rlo + e) - t0) : __ldcg(A.rec_k + rlo + e); };   // (m > EV_MAX only)
     const TileAgg g = tb.ag;
     int pend, nwin0, tok0;
     int64_t T0;
     if (!DENSE) {
-        const Pre X = look_back(A, tile, lane);
+        bool ready;
         Agg ga; ga.hasev = g.hasev; ga.fk = g.fk; ga.lk = g.lk; ga.closed = g.closed; ga.tn = g.tn; ga.tail = g.tail;
+        const Pre X = look_back(A, tile, ga, lane, force, ready);
+        if (!ready) return false;
         pend = P.mode == MODE_KMER ? X.o.r : 0;
         const int nbase0 = pend + g.fk;
         nwin0 = (int)div_k((uint32_t)nbase0, P);
@@ -200,24 +222,13 @@ __device__ __forceinline__ void scan_tables(const EncArgs &A, const Smem7 &sm, T
                                         (uint32_t)Y.o.r | ((uint32_t)Y.cnt << 4) | ((uint32_t)(Y.tail >> 32) << 8)));
             st_vol128(&D.i1, make_uint4(tagI, (uint32_t)Y.o.q, (uint32_t)((uint64_t)Y.o.q >> 32), (uint32_t)Y.tail));
         }
-        // carried bases of the open record go in front of region 0
-        uint32_t cw = 0, fw = 0;
-        if (lane < pend) {
-            const uint32_t c = (uint32_t)(X.tail >> (3 * (pend - 1 - lane))) & 7u;
-            const int uu = PEND - pend + lane;
-            const uint32_t dg = c < CLS_N ? c : (c == CLS_N ? 2u : 1u);
-            cw = dg << (30 - 2 * (uu & 15));
-            fw = c >= CLS_N ? (1u << (31 - (uu & 31))) : 0u;
-        }
-        cw = __reduce_or_sync(FULL, cw); fw = __reduce_or_sync(FULL, fw);
-        if (lane == 0) { st[(PEND >> 4) - 1] = cw; st[SW_CODE + (PEND >> 5) - 1] = fw; }
+        // carried bases of the open record go right in front of region 0's first kept base
+        if (lane < pend) put_class(st, tb.rbase[0] - pend + lane, (uint32_t)(X.tail >> (3 * (pend - 1 - lane))) & 7u);
         T0 = A.out_bias + X.T + X.o.q;
     } else {
         // closed form: the open record started at a known byte, every byte before the tile is a kept base
-        const int64_t rlo = tb.rlo;
         pend = 0; nwin0 = 0; tok0 = 0;
         T0 = rlo <= A.n_rec ? __ldg(A.out_off + (rlo > 0 ? rlo - 1 : 0)) : 0;
-        uint32_t cw = 0, fw = 0;
         if (rlo > 0) {
             const int64_t nb = t0 - rec_pos(A, rlo - 1);
             const int64_t q = nb / k;
@@ -226,22 +237,11 @@ __device__ __forceinline__ void scan_tables(const EncArgs &A, const Smem7 &sm, T
             const int nbase0 = pend + g.fk;
             nwin0 = (int)div_k((uint32_t)nbase0, P);
             tok0 = nwin0 + (g.hasev ? tail_tokens(nbase0 - nwin0 * k, P) : 0);
-            if (lane < pend) {
-                const uint32_t c = sm.lut[__ldg(A.bytes_al + t0 - pend + lane)];
-                const int uu = PEND - pend + lane;
-                const uint32_t dg = c < CLS_N ? c : (c == CLS_N ? 2u : 1u);
-                cw = dg << (30 - 2 * (uu & 15));
-                fw = c >= CLS_N ? (1u << (31 - (uu & 31))) : 0u;
-            }
+            if (lane < pend) put_class(st, tb.rbase[0] - pend + lane, sm.lut[__ldg(A.bytes_al + t0 - pend + lane)]);
         }
-        cw = __reduce_or_sync(FULL, cw); fw = __reduce_or_sync(FULL, fw);
-        if (lane == 0) { st[(PEND >> 4) - 1] = cw; st[SW_CODE + (PEND >> 5) - 1] = fw; }
     }
     const int ntok = tb.ntok + tok0;
-    if (lane == 0) {
-        tb.T0 = T0; tb.ntok = ntok; tb.pend = pend; tb.tok0 = tok0; tb.nwin0 = nwin0;
-        tb.e_tile = tile; tb.e_m = m; tb.e_rlo = tb.rlo;
-    }
+    if (lane == 0) { tb.T0 = T0; tb.ntok = ntok; tb.pend = pend; tb.tok0 = tok0; tb.nwin0 = nwin0; }
     __syncwarp();
     if (m > EV_MAX) {
         // per-token fallback emission: only out_offsets are prepared here (records that start inside the tile)
@@ -249,9 +249,9 @@ __device__ __forceinline__ void scan_tables(const EncArgs &A, const Smem7 &sm, T
             long long carry = T0 + tok0;
             for (int c0 = 0; c0 < m; c0 += 32) {
                 const int e = c0 + lane;
-                const int ke = e < m ? event_kept<DENSE>(A, tb, e, t0) : ktot;
+                const int ke = e < m ? kept(e) : ktot;
                 int kn = __shfl_down_sync(FULL, ke, 1);
-                if (lane == 31) kn = e + 1 < m ? event_kept<DENSE>(A, tb, e + 1, t0) : ktot;
+                if (lane == 31) kn = e + 1 < m ? kept(e + 1) : ktot;
                 if (e >= m - 1) kn = ktot;
                 const int ne = e < m ? kn - ke : 0;
                 const int nw = (int)div_k((uint32_t)ne, P);
@@ -259,7 +259,7 @@ __device__ __forceinline__ void scan_tables(const EncArgs &A, const Smem7 &sm, T
                 int ti = te;
 #pragma unroll
                 for (int d = 1; d < 32; d <<= 1) { const int t = __shfl_up_sync(FULL, ti, d); if (lane >= d) ti += t; }
-                if (e < m) A.out_off[tb.rlo + e] = carry + ti - te;
+                if (e < m) A.out_off[rlo + e] = carry + ti - te;
                 carry += __shfl_sync(FULL, ti, 31);
             }
             __threadfence();
@@ -269,7 +269,7 @@ __device__ __forceinline__ void scan_tables(const EncArgs &A, const Smem7 &sm, T
         for (int e = lane; e < m; e += 32) {
             const int t = tb.le_t[1 + e] + tok0;
             tb.le_t[1 + e] = t;
-            if (!DENSE) A.out_off[tb.rlo + e] = T0 + t;
+            if (!DENSE) A.out_off[rlo + e] = T0 + t;
         }
         if (lane == 0) { tb.le_src[0] = -pend; tb.le_t[0] = 0; tb.le_nwin[0] = nwin0; tb.le_t[m + 1] = ntok; }
         __syncwarp();
@@ -282,13 +282,13 @@ __device__ __forceinline__ void scan_tables(const EncArgs &A, const Smem7 &sm, T
 #pragma unroll
                 for (int w = 1; w < NWC; ++w) reg += (tb.cum[w] <= ls) ? 1 : 0;
                 const int rank = j + reg;
-                tb.se_src[rank] = reg_slot(reg) + (ls - tb.cum[reg]);
+                tb.se_src[rank] = tb.rbase[reg] + (ls - tb.cum[reg]);
                 tb.se_t[rank] = tb.le_t[j];
                 tb.se_nwin[rank] = tb.le_nwin[j];
             }
         }
         if (lane == 0) {
-            tb.se_src[0] = PEND - pend; tb.se_t[0] = 0; tb.se_nwin[0] = nwin0;
+            tb.se_src[0] = tb.rbase[0] - pend; tb.se_t[0] = 0; tb.se_nwin[0] = nwin0;
             tb.reg_e0[0] = 0; tb.reg_e0[NWC] = m + NWC; tb.se_t[m + NWC] = ntok;
         } else if (lane < NWC) {
             const int c = tb.cum[lane];
@@ -308,7 +308,7 @@ __device__ __forceinline__ void scan_tables(const EncArgs &A, const Smem7 &sm, T
                 ls = src + nwj * k + i; t = tj + nwj + min(i, nt); nw = 0;
             }
             const int rank = lane + lo;
-            tb.se_src[rank] = reg_slot(lane) + (ls - c);
+            tb.se_src[rank] = tb.rbase[lane] + (ls - c);
             tb.se_t[rank] = t;
             tb.se_nwin[rank] = nw;
             tb.reg_e0[lane] = rank;
@@ -322,12 +322,13 @@ __device__ __forceinline__ void scan_tables(const EncArgs &A, const Smem7 &sm, T
         if (u < ktot) {
             const int s = slot_of(tb, u);
             const uint32_t dg = code_at(st, s, 1), fl = flags_at(st, s, 1);
-            const int dst = reg_slot(w) + (tb.cum[w + 1] - tb.cum[w]) + i;
+            const int dst = tb.rbase[w] + (tb.cum[w + 1] - tb.cum[w]) + i;
             if (dg) atomicOr(&st[dst >> 4], dg << (30 - 2 * (dst & 15)));
             if (fl) atomicOr(&st[SW_CODE + (dst >> 5)], 1u << (31 - (dst & 31)));
         }
     }
     __syncwarp();
+    return true;
 }
 
 // ---- per-token fallback emission of a tile with more record starts than the tables hold (all compute threads) -----
