@@ -1,7 +1,7 @@
 // dnatok_api.cu -- host side of the C-ABI declared in include/dnatok.h.
 //
 // Argument marshalling, scratch management and the pinned multi-stream scheduler; every
-// step of the hot path itself runs in the kernels of encode_v7.cuh / bpe_kernel.cuh /
+// step of the hot path itself runs in the kernels of encode_v5.cuh / encode_v7.cuh / bpe_kernel.cuh /
 // pad_kernel.cuh.  There is no CPU fallback anywhere in this file.
 #include "../../include/dnatok.h"
 
@@ -14,6 +14,7 @@
 
 #include "bpe_kernel.cuh"
 #include "common.cuh"
+#include "encode_v5.cuh"
 #include "encode_v7.cuh"
 #include "pad_kernel.cuh"
 
@@ -73,7 +74,7 @@ struct dnatok {
     int32_t bpe_cap = 0;
     EncCtx ctx;
     StreamRing ring;
-    int enc_ctas_per_sm = 1, bpe_ctas_per_sm = 1;
+    int enc_ctas_per_sm = 1, dense_ctas_per_sm = 1, bpe_ctas_per_sm = 1;
     bool dense = false;                // no SKIP class and strip_headers == 0: kept bases = bytes, the no-scan encoder runs
     int force_S = 0;                   // dnatok_set_super_tile: fixed super-tile size in sub-tiles (0 = automatic)
     int grid_cap = 0;                  // dnatok_set_grid_cap: at most this many persistent CTAs per launch (0 = no cap)
@@ -167,20 +168,36 @@ int ctx_next_gen(dnatok_t *h, EncCtx &c, cudaStream_t st) {
     return DNATOK_OK;
 }
 
-template <typename IdT, bool DENSE>
-void launch_variant(const EncArgs &a, int kk, int grid, cudaStream_t st) {
-    // the headline shapes get a kernel with only their own emission variant compiled in (smaller instruction footprint)
+// the headline shapes get a kernel with only their own emission variant compiled in (smaller instruction footprint)
+template <typename IdT>
+void launch_dense(const EncArgs &a, int kk, int grid, cudaStream_t st) {
     constexpr bool wide = sizeof(IdT) >= 2;                    // uint8 ids: the BPE class pass, single-nt only
     switch (wide ? kk : 0) {
-        case 0: encode_tiles_v7<IdT, 0, DENSE><<<grid, NT7, sizeof(Smem7), st>>>(a); break;
-        case 1: encode_tiles_v7<IdT, wide ? 1 : 0, DENSE><<<grid, NT7, sizeof(Smem7), st>>>(a); break;
-        case 2: encode_tiles_v7<IdT, wide ? 2 : 0, DENSE><<<grid, NT7, sizeof(Smem7), st>>>(a); break;
-        case 3: encode_tiles_v7<IdT, wide ? 3 : 0, DENSE><<<grid, NT7, sizeof(Smem7), st>>>(a); break;
-        case 4: encode_tiles_v7<IdT, wide ? 4 : 0, DENSE><<<grid, NT7, sizeof(Smem7), st>>>(a); break;
-        case 5: encode_tiles_v7<IdT, wide ? 5 : 0, DENSE><<<grid, NT7, sizeof(Smem7), st>>>(a); break;
-        case 6: encode_tiles_v7<IdT, wide ? 6 : 0, DENSE><<<grid, NT7, sizeof(Smem7), st>>>(a); break;
-        case 8: encode_tiles_v7<IdT, wide ? 8 : 0, DENSE><<<grid, NT7, sizeof(Smem7), st>>>(a); break;
-        default: encode_tiles_v7<IdT, wide ? -1 : 0, DENSE><<<grid, NT7, sizeof(Smem7), st>>>(a); break;
+        case 0: v7::encode_tiles_v7<IdT, 0, true><<<grid, v7::NT7, sizeof(v7::Smem7), st>>>(a); break;
+        case 1: v7::encode_tiles_v7<IdT, wide ? 1 : 0, true><<<grid, v7::NT7, sizeof(v7::Smem7), st>>>(a); break;
+        case 2: v7::encode_tiles_v7<IdT, wide ? 2 : 0, true><<<grid, v7::NT7, sizeof(v7::Smem7), st>>>(a); break;
+        case 3: v7::encode_tiles_v7<IdT, wide ? 3 : 0, true><<<grid, v7::NT7, sizeof(v7::Smem7), st>>>(a); break;
+        case 4: v7::encode_tiles_v7<IdT, wide ? 4 : 0, true><<<grid, v7::NT7, sizeof(v7::Smem7), st>>>(a); break;
+        case 5: v7::encode_tiles_v7<IdT, wide ? 5 : 0, true><<<grid, v7::NT7, sizeof(v7::Smem7), st>>>(a); break;
+        case 6: v7::encode_tiles_v7<IdT, wide ? 6 : 0, true><<<grid, v7::NT7, sizeof(v7::Smem7), st>>>(a); break;
+        case 8: v7::encode_tiles_v7<IdT, wide ? 8 : 0, true><<<grid, v7::NT7, sizeof(v7::Smem7), st>>>(a); break;
+        default: v7::encode_tiles_v7<IdT, wide ? -1 : 0, true><<<grid, v7::NT7, sizeof(v7::Smem7), st>>>(a); break;
+    }
+}
+template <typename IdT>
+void launch_strip(const EncArgs &a, int kk, int grid, cudaStream_t st) {
+    using namespace dtk::v5;
+    constexpr bool wide = sizeof(IdT) >= 2;
+    switch (wide ? kk : 0) {
+        case 0: encode_tiles_v5<IdT, 0><<<grid, NT, sizeof(Smem5), st>>>(a); break;
+        case 1: encode_tiles_v5<IdT, wide ? 1 : 0><<<grid, NT, sizeof(Smem5), st>>>(a); break;
+        case 2: encode_tiles_v5<IdT, wide ? 2 : 0><<<grid, NT, sizeof(Smem5), st>>>(a); break;
+        case 3: encode_tiles_v5<IdT, wide ? 3 : 0><<<grid, NT, sizeof(Smem5), st>>>(a); break;
+        case 4: encode_tiles_v5<IdT, wide ? 4 : 0><<<grid, NT, sizeof(Smem5), st>>>(a); break;
+        case 5: encode_tiles_v5<IdT, wide ? 5 : 0><<<grid, NT, sizeof(Smem5), st>>>(a); break;
+        case 6: encode_tiles_v5<IdT, wide ? 6 : 0><<<grid, NT, sizeof(Smem5), st>>>(a); break;
+        case 8: encode_tiles_v5<IdT, wide ? 8 : 0><<<grid, NT, sizeof(Smem5), st>>>(a); break;
+        default: encode_tiles_v5<IdT, wide ? -1 : 0><<<grid, NT, sizeof(Smem5), st>>>(a); break;
     }
 }
 
@@ -193,18 +210,19 @@ int launch_tiles(dnatok_t *h, EncCtx &c, const EncParams &prm, const uint8_t *d_
     a.mis = (int64_t)(addr & 15);
     a.bytes_al = reinterpret_cast<const uint8_t *>(addr - (uintptr_t)a.mis);
     a.p_end = a.mis + n_bytes;
-    // tile size: large inputs want large tiles (the per-tile work of the scan warp is amortised over S x 16 KiB);
-    // small inputs want enough tiles to occupy every CTA slot a few times over; inputs with many short records want
-    // few record starts per tile (the segment tables hold EV_MAX)
-    const int64_t slots = (int64_t)h->sm_count * h->enc_ctas_per_sm;
+    // tile size: large inputs want large tiles (the per-tile scan work is amortised over S x 16 KiB); small inputs
+    // want enough tiles to occupy every CTA slot a few times over; the no-scan encoder also wants few record starts
+    // per tile (its segment tables hold v7::EV_MAX)
+    const bool dense = h->dense;
+    const int64_t slots = (int64_t)h->sm_count * (dense ? h->dense_ctas_per_sm : h->enc_ctas_per_sm);
     int S = S_MAX;
     while (S > 1 && a.p_end / ((int64_t)S * TB) + 1 < 3 * slots) S >>= 1;
-    while (S > 1 && n_rec * (int64_t)S * TB > (EV_MAX / 2) * std::max<int64_t>(n_bytes, 1)) S >>= 1;
+    while (dense && S > 1 && n_rec * (int64_t)S * TB > (v7::EV_MAX / 2) * std::max<int64_t>(n_bytes, 1)) S >>= 1;
     if (h->force_S > 0) S = h->force_S;
     a.S = S;
     int64_t n_tiles = a.p_end / ((int64_t)S * TB) + 1;
     if (n_tiles > 0x7fffffff) return fail(h, DNATOK_EINVAL, "n_bytes too large for one call");
-    const int64_t n_scan_blocks = h->dense ? (n_rec + DS_BLK - 1) / DS_BLK + (n_rec == 0) : 0;
+    const int64_t n_scan_blocks = dense ? (n_rec + v7::DS_BLK - 1) / v7::DS_BLK + (n_rec == 0) : 0;
     int rc = ctx_reserve_tiles(h, c, std::max(n_tiles, n_scan_blocks), n_rec, st); if (rc) return rc;
     rc = ctx_next_gen(h, c, st); if (rc) return rc;
     a.rec_off = d_rec_off; a.n_rec = n_rec; a.off_bias = off_bias;
@@ -213,17 +231,17 @@ int launch_tiles(dnatok_t *h, EncCtx &c, const EncParams &prm, const uint8_t *d_
     a.status = c.d_status; a.prof = c.prof; a.gen = c.gen; a.n_tiles = (int32_t)n_tiles; a.prm = prm;
     int grid = (int)std::min<int64_t>(n_tiles, slots);
     if (h->grid_cap > 0) grid = std::min(grid, h->grid_cap);
-    tile_first_rec_kernel<<<(unsigned)((n_tiles + 1 + 255) / 256), 256, 0, st>>>(a);
+    v7::tile_first_rec_kernel<<<(unsigned)((n_tiles + 1 + 255) / 256), 256, 0, st>>>(a);
     CU(cudaGetLastError());
     h->launches += 1;
     const int kk = prm.mode == MODE_KMER ? prm.k : 0;
-    if (h->dense) {
-        dense_offsets_kernel<<<(unsigned)n_scan_blocks, DS_NT, 0, st>>>(a, c.descs);
+    if (dense) {
+        v7::dense_offsets_kernel<<<(unsigned)n_scan_blocks, v7::DS_NT, 0, st>>>(a, c.descs);
         CU(cudaGetLastError());
         h->launches += 1;
-        launch_variant<IdT, true>(a, kk, grid, st);
+        launch_dense<IdT>(a, kk, grid, st);
     } else {
-        launch_variant<IdT, false>(a, kk, grid, st);
+        launch_strip<IdT>(a, kk, grid, st);
     }
     CU(cudaGetLastError());
     c.ticket_base += (unsigned long long)n_tiles + (unsigned long long)grid;
@@ -474,20 +492,28 @@ int dnatok_create(const dnatok_config *cfg_in, int device, dnatok_t **out) {
         h->bpe_ctas_per_sm = std::max(nb, 1);
     }
     {
-        // the streams of two tiles need more than the default 48 KiB of shared memory per CTA
-#define DTK_VARIANTS(T, D) (const void *)encode_tiles_v7<T, 0, D>, (const void *)encode_tiles_v7<T, 1, D>, (const void *)encode_tiles_v7<T, 2, D>, \
-                           (const void *)encode_tiles_v7<T, 3, D>, (const void *)encode_tiles_v7<T, 4, D>, (const void *)encode_tiles_v7<T, 5, D>, \
-                           (const void *)encode_tiles_v7<T, 6, D>, (const void *)encode_tiles_v7<T, 8, D>, (const void *)encode_tiles_v7<T, -1, D>
-        const void *kernels[] = {DTK_VARIANTS(int32_t, false), DTK_VARIANTS(int16_t, false), DTK_VARIANTS(int32_t, true),
-                                 DTK_VARIANTS(int16_t, true), (const void *)encode_tiles_v7<uint8_t, 0, false>,
-                                 (const void *)encode_tiles_v7<uint8_t, 0, true>};
-#undef DTK_VARIANTS
-        for (const void *kf : kernels)
-            if (cudaFuncSetAttribute(kf, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Smem7)) != cudaSuccess)
+        // both encoders need more than the default 48 KiB of shared memory per CTA
+#define DTK_V5(T) (const void *)v5::encode_tiles_v5<T, 0>, (const void *)v5::encode_tiles_v5<T, 1>, (const void *)v5::encode_tiles_v5<T, 2>, \
+                  (const void *)v5::encode_tiles_v5<T, 3>, (const void *)v5::encode_tiles_v5<T, 4>, (const void *)v5::encode_tiles_v5<T, 5>, \
+                  (const void *)v5::encode_tiles_v5<T, 6>, (const void *)v5::encode_tiles_v5<T, 8>, (const void *)v5::encode_tiles_v5<T, -1>
+#define DTK_V7(T) (const void *)v7::encode_tiles_v7<T, 0, true>, (const void *)v7::encode_tiles_v7<T, 1, true>, (const void *)v7::encode_tiles_v7<T, 2, true>, \
+                  (const void *)v7::encode_tiles_v7<T, 3, true>, (const void *)v7::encode_tiles_v7<T, 4, true>, (const void *)v7::encode_tiles_v7<T, 5, true>, \
+                  (const void *)v7::encode_tiles_v7<T, 6, true>, (const void *)v7::encode_tiles_v7<T, 8, true>, (const void *)v7::encode_tiles_v7<T, -1, true>
+        const void *k5[] = {DTK_V5(int32_t), DTK_V5(int16_t), (const void *)v5::encode_tiles_v5<uint8_t, 0>};
+        const void *k7[] = {DTK_V7(int32_t), DTK_V7(int16_t), (const void *)v7::encode_tiles_v7<uint8_t, 0, true>};
+#undef DTK_V5
+#undef DTK_V7
+        for (const void *kf : k5)
+            if (cudaFuncSetAttribute(kf, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(v5::Smem5)) != cudaSuccess)
+                return bail(DNATOK_ECUDA);
+        for (const void *kf : k7)
+            if (cudaFuncSetAttribute(kf, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(v7::Smem7)) != cudaSuccess)
                 return bail(DNATOK_ECUDA);
         int nb = 0;
-        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, encode_tiles_v7<int32_t, -1, false>, NT7, sizeof(Smem7));
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, v5::encode_tiles_v5<int32_t, -1>, NT, sizeof(v5::Smem5));
         h->enc_ctas_per_sm = std::max(nb, 1);
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, v7::encode_tiles_v7<int32_t, -1, true>, v7::NT7, sizeof(v7::Smem7));
+        h->dense_ctas_per_sm = std::max(nb, 1);
         h->dense = !cfg.strip_headers;
         for (int b = 0; b < 256; ++b) if (cfg.class_lut[b] == DNATOK_CLS_SKIP) h->dense = false;
     }

@@ -30,6 +30,7 @@
 #include "common.cuh"
 
 namespace dtk {
+namespace v7 {
 
 constexpr int NWC = NT / 32;                 // compute warps
 static_assert(NWC == 8, "eight regions per tile");
@@ -666,6 +667,7 @@ __device__ __noinline__ Pre look_back(const EncArgs &A, int tile, const Agg &own
     return pre_extend(X, G, P);                          // walked back to the very beginning
 }
 
+}  // namespace v7
 }  // namespace dtk
 
 #include "encode_v7_compact.cuh"

@@ -3,6 +3,7 @@
 #pragma once
 
 namespace dtk {
+namespace v7 {
 
 // byte q (0..63) of this lane's staged 64 bytes
 __device__ __forceinline__ uint32_t staged_byte(const uint4 *slot, int q) {
@@ -445,4 +446,5 @@ __device__ __forceinline__ void compact_region(const EncArgs &A, Smem7 &sm, Tile
     }
 }
 
+}  // namespace v7
 }  // namespace dtk

@@ -2,6 +2,7 @@
 #pragma once
 
 namespace dtk {
+namespace v7 {
 
 #ifdef DTK_PROF
 #define PROF_T(var) const long long var = clock64()
@@ -141,4 +142,5 @@ __global__ void __launch_bounds__(NT7, 3) encode_tiles_v7(const __grid_constant_
     }
 }
 
+}  // namespace v7
 }  // namespace dtk

@@ -3,6 +3,7 @@
 #pragma once
 
 namespace dtk {
+namespace v7 {
 
 // ---- preparation of a tile: record range, record-start list, L2 prefetch ------------------------------------------
 __device__ __forceinline__ int scan_prep(const EncArgs &A, TileBuf &tb, unsigned long long ticket, int lane) {
@@ -375,4 +376,5 @@ __device__ __noinline__ void emit_generic(const EncArgs &A, const uint32_t *st, 
     }
 }
 
+}  // namespace v7
 }  // namespace dtk
