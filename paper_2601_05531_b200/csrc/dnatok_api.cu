@@ -231,16 +231,18 @@ int launch_tiles(dnatok_t *h, EncCtx &c, const EncParams &prm, const uint8_t *d_
     a.status = c.d_status; a.prof = c.prof; a.gen = c.gen; a.n_tiles = (int32_t)n_tiles; a.prm = prm;
     int grid = (int)std::min<int64_t>(n_tiles, slots);
     if (h->grid_cap > 0) grid = std::min(grid, h->grid_cap);
-    v7::tile_first_rec_kernel<<<(unsigned)((n_tiles + 1 + 255) / 256), 256, 0, st>>>(a);
-    CU(cudaGetLastError());
-    h->launches += 1;
     const int kk = prm.mode == MODE_KMER ? prm.k : 0;
+    const unsigned nb_first = (unsigned)((n_tiles + 1 + 255) / 256);
     if (dense) {
-        v7::dense_offsets_kernel<<<(unsigned)n_scan_blocks, v7::DS_NT, 0, st>>>(a, c.descs);
+        // record range of every tile + out_offsets (closed form from the record lengths), one launch
+        v7::dense_prepass_kernel<<<nb_first + (unsigned)n_scan_blocks, v7::DS_NT, 0, st>>>(a, c.descs, (int)nb_first);
         CU(cudaGetLastError());
         h->launches += 1;
         launch_dense<IdT>(a, kk, grid, st);
     } else {
+        v5::tile_first_rec_kernel<<<nb_first, 256, 0, st>>>(a);
+        CU(cudaGetLastError());
+        h->launches += 1;
         launch_strip<IdT>(a, kk, grid, st);
     }
     CU(cudaGetLastError());

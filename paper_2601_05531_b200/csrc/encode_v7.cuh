@@ -452,22 +452,6 @@ __device__ __forceinline__ void emit_region(const EncArgs &A, const uint32_t *st
 
 // ---- pre-pass ---------------------------------------------------------------------------------------------
 // first_rec[t] = first r in [0, n_rec] with position >= t * S * TB (n_rec + 1 if none); first_rec[n_tiles] = n_rec + 1
-__global__ void __launch_bounds__(256) tile_first_rec_kernel(const __grid_constant__ EncArgs A) {
-    const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (t > A.n_tiles) return;
-    int64_t lo = 0, hi = A.n_rec + 1;
-    if (t < A.n_tiles) {
-        const int64_t pos = t * A.S * TB;
-        while (lo < hi) {
-            const int64_t mid = (lo + hi) >> 1;
-            if (rec_pos(A, mid) >= pos) hi = mid; else lo = mid + 1;
-        }
-    } else {
-        lo = A.n_rec + 1;
-    }
-    A.first_rec[t] = lo;
-}
-
 __device__ __forceinline__ void prefetch_l2(const EncArgs &A, int64_t b0, int bytes) {   // [b0, b0 + bytes) clipped to the input
     int64_t sz = A.p_end - b0;
     sz = sz >= bytes ? bytes : ((sz + 15) & ~(int64_t)15);
@@ -484,11 +468,27 @@ __device__ __forceinline__ int64_t dense_tokens(int64_t len, const EncParams &P)
     const int64_t q = len / P.k;
     return q + tail_tokens((int)(len - q * P.k), P);
 }
-__global__ void __launch_bounds__(DS_NT) dense_offsets_kernel(const __grid_constant__ EncArgs A, TileDesc *chain) {
+// One launch: blocks [0, nb_first) write first_rec (256 tiles each), the blocks behind them run the offsets scan.
+__global__ void __launch_bounds__(DS_NT) dense_prepass_kernel(const __grid_constant__ EncArgs A, TileDesc *chain, int nb_first) {
     __shared__ long long wsum[DS_NT / 32];
     __shared__ long long s_base;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int64_t r0 = (int64_t)blockIdx.x * DS_BLK + (int64_t)tid * DS_PER;
+    if ((int)blockIdx.x < nb_first) {
+        const int64_t t = (int64_t)blockIdx.x * DS_NT + tid;
+        if (t > A.n_tiles) return;
+        int64_t lo = 0, hi = A.n_rec + 1;
+        if (t < A.n_tiles) {
+            const int64_t pos = t * A.S * TB;
+            while (lo < hi) {
+                const int64_t mid = (lo + hi) >> 1;
+                if (rec_pos(A, mid) >= pos) hi = mid; else lo = mid + 1;
+            }
+        } else lo = A.n_rec + 1;
+        A.first_rec[t] = lo;
+        return;
+    }
+    const int b = (int)blockIdx.x - nb_first;
+    const int64_t r0 = (int64_t)b * DS_BLK + (int64_t)tid * DS_PER;
     long long v[DS_PER], run = 0;
 #pragma unroll
     for (int i = 0; i < DS_PER; ++i) {
@@ -506,7 +506,6 @@ __global__ void __launch_bounds__(DS_NT) dense_offsets_kernel(const __grid_const
     for (int w = 0; w < DS_NT / 32; ++w) { const long long t = wsum[w]; if (w < warp) woff += t; tot += t; }
     const uint32_t tagA = (A.gen << 2) | ST_AGG, tagI = (A.gen << 2) | ST_INCL;
     if (tid == 0) {
-        const int b = blockIdx.x;
         long long base = 0;
         if (b > 0) {
             st_vol128(&chain[b].a0, make_uint4(tagA, 0u, (uint32_t)tot, (uint32_t)((unsigned long long)tot >> 32)));
