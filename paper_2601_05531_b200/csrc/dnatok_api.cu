@@ -8,7 +8,6 @@
 #include <algorithm>
 #include <cstdarg>
 #include <cstdio>
-#include <cstdlib>
 #include <cstring>
 #include <string>
 #include <vector>
@@ -17,7 +16,6 @@
 #include "common.cuh"
 #include "encode_v5.cuh"
 #include "encode_v7.cuh"
-#include "encode_v8.cuh"
 #include "pad_kernel.cuh"
 
 using namespace dtk;
@@ -79,7 +77,6 @@ struct dnatok {
     int enc_ctas_per_sm = 1, dense_ctas_per_sm = 1, bpe_ctas_per_sm = 1;
     bool dense = false;                // no SKIP class and strip_headers == 0: kept bases = bytes, the no-scan encoder runs
     int force_S = 0;                   // dnatok_set_super_tile: fixed super-tile size in sub-tiles (0 = automatic)
-    int encoder = 8;                   // strip path: 8 = encode_v8.cuh, 5 = encode_v5.cuh (env DTK_ENCODER, A/B runs only)
     int grid_cap = 0;                  // dnatok_set_grid_cap: at most this many persistent CTAs per launch (0 = no cap)
     int64_t launches = 0;
     std::string err;
@@ -188,22 +185,6 @@ void launch_dense(const EncArgs &a, int kk, int grid, cudaStream_t st) {
     }
 }
 template <typename IdT>
-void launch_strip8(const EncArgs &a, int kk, int grid, cudaStream_t st) {
-    using namespace dtk::v8;
-    constexpr bool wide = sizeof(IdT) >= 2;
-    switch (wide ? kk : 0) {
-        case 0: encode_tiles_v8<IdT, 0><<<grid, NT, sizeof(Smem8), st>>>(a); break;
-        case 1: encode_tiles_v8<IdT, wide ? 1 : 0><<<grid, NT, sizeof(Smem8), st>>>(a); break;
-        case 2: encode_tiles_v8<IdT, wide ? 2 : 0><<<grid, NT, sizeof(Smem8), st>>>(a); break;
-        case 3: encode_tiles_v8<IdT, wide ? 3 : 0><<<grid, NT, sizeof(Smem8), st>>>(a); break;
-        case 4: encode_tiles_v8<IdT, wide ? 4 : 0><<<grid, NT, sizeof(Smem8), st>>>(a); break;
-        case 5: encode_tiles_v8<IdT, wide ? 5 : 0><<<grid, NT, sizeof(Smem8), st>>>(a); break;
-        case 6: encode_tiles_v8<IdT, wide ? 6 : 0><<<grid, NT, sizeof(Smem8), st>>>(a); break;
-        case 8: encode_tiles_v8<IdT, wide ? 8 : 0><<<grid, NT, sizeof(Smem8), st>>>(a); break;
-        default: encode_tiles_v8<IdT, wide ? -1 : 0><<<grid, NT, sizeof(Smem8), st>>>(a); break;
-    }
-}
-template <typename IdT>
 void launch_strip(const EncArgs &a, int kk, int grid, cudaStream_t st) {
     using namespace dtk::v5;
     constexpr bool wide = sizeof(IdT) >= 2;
@@ -262,8 +243,7 @@ int launch_tiles(dnatok_t *h, EncCtx &c, const EncParams &prm, const uint8_t *d_
         v5::tile_first_rec_kernel<<<nb_first, 256, 0, st>>>(a);
         CU(cudaGetLastError());
         h->launches += 1;
-        if (h->encoder == 8) launch_strip8<IdT>(a, kk, grid, st);
-        else launch_strip<IdT>(a, kk, grid, st);
+        launch_strip<IdT>(a, kk, grid, st);
     }
     CU(cudaGetLastError());
     c.ticket_base += (unsigned long long)n_tiles + (unsigned long long)grid;
@@ -523,15 +503,6 @@ int dnatok_create(const dnatok_config *cfg_in, int device, dnatok_t **out) {
                   (const void *)v7::encode_tiles_v7<T, 6, true>, (const void *)v7::encode_tiles_v7<T, 8, true>, (const void *)v7::encode_tiles_v7<T, -1, true>
         const void *k5[] = {DTK_V5(int32_t), DTK_V5(int16_t), (const void *)v5::encode_tiles_v5<uint8_t, 0>};
         const void *k7[] = {DTK_V7(int32_t), DTK_V7(int16_t), (const void *)v7::encode_tiles_v7<uint8_t, 0, true>};
-#define DTK_V8(T) (const void *)v8::encode_tiles_v8<T, 0>, (const void *)v8::encode_tiles_v8<T, 1>, (const void *)v8::encode_tiles_v8<T, 2>, \
-                  (const void *)v8::encode_tiles_v8<T, 3>, (const void *)v8::encode_tiles_v8<T, 4>, (const void *)v8::encode_tiles_v8<T, 5>, \
-                  (const void *)v8::encode_tiles_v8<T, 6>, (const void *)v8::encode_tiles_v8<T, 8>, (const void *)v8::encode_tiles_v8<T, -1>
-        const void *k8[] = {DTK_V8(int32_t), DTK_V8(int16_t), (const void *)v8::encode_tiles_v8<uint8_t, 0>};
-#undef DTK_V8
-        for (const void *kf : k8)
-            if (cudaFuncSetAttribute(kf, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(v8::Smem8)) != cudaSuccess)
-                return bail(DNATOK_ECUDA);
-        if (const char *e = getenv("DTK_ENCODER")) h->encoder = atoi(e) == 5 ? 5 : 8;
 #undef DTK_V5
 #undef DTK_V7
         for (const void *kf : k5)
@@ -543,10 +514,6 @@ int dnatok_create(const dnatok_config *cfg_in, int device, dnatok_t **out) {
         int nb = 0;
         cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, v5::encode_tiles_v5<int32_t, -1>, NT, sizeof(v5::Smem5));
         h->enc_ctas_per_sm = std::max(nb, 1);
-        if (h->encoder == 8) {
-            cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, v8::encode_tiles_v8<int32_t, -1>, NT, sizeof(v8::Smem8));
-            h->enc_ctas_per_sm = std::max(nb, 1);
-        }
         cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, v7::encode_tiles_v7<int32_t, -1, true>, v7::NT7, sizeof(v7::Smem7));
         h->dense_ctas_per_sm = std::max(nb, 1);
         h->dense = !cfg.strip_headers;

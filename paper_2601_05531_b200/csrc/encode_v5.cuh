@@ -490,8 +490,7 @@ __device__ __forceinline__ void prefetch_l2(const EncArgs &A, int64_t b0) {     
 }
 
 // ---- next-super-tile preparation (one warp): record range, record-start list, entry line state, L2 prefetch ----
-template <typename SM>
-__device__ __forceinline__ void prep_super(const EncArgs &A, SM &sm, int par, unsigned long long ticket, int lane,
+__device__ __forceinline__ void prep_super(const EncArgs &A, Smem5 &sm, int par, unsigned long long ticket, int lane,
                                            int64_t pos_first, int64_t pos_last) {
     constexpr uint32_t FULL = 0xffffffffu;
     const unsigned long long rel = ticket - A.ticket_base;
@@ -547,8 +546,7 @@ __device__ __forceinline__ void prep_super(const EncArgs &A, SM &sm, int par, un
 }
 
 // exclusive block scan of one int per thread (two barriers)
-template <typename SM>
-__device__ __forceinline__ int block_exscan5(int v, SM &sm, int &total) {
+__device__ __forceinline__ int block_exscan5(int v, Smem5 &sm, int &total) {
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     int inc = v;
 #pragma unroll
