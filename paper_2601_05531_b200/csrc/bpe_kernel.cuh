@@ -1,38 +1,77 @@
-// bpe_kernel.cuh -- BPE merge kernel: one read per thread block, lowest rank first.
+// bpe_kernel.cuh -- BPE merges, organised around ACGT SEGMENTS, lowest rank first.
 //
-// Semantics: the kept classes of a read are cut at every
-// N / UNK (each is its own token and a hard boundary); inside each ACGT segment, repeat
-// { take the lowest-rank adjacent pair that has a rule; replace all its occurrences left to
-// right without overlap } until no adjacent pair has a rule.
+// Semantics: the kept classes of a read are cut at every N / UNK (each is its own token
+// and a hard boundary); inside each ACGT segment, repeat { take the lowest-rank adjacent pair that has a rule; replace
+// all its occurrences left to right without overlap } until no adjacent pair has a rule.  For a valid table (rule r's
+// parts are tokens < 4 + r) this equals applying ONE occurrence at a time in (rank, position) order: a merge of rank m
+// only creates pairs of rank > m, so the minimum never decreases and equal ranks are met left to right.  That is the
+// form used here.
 //
-// Parallel form: all segments of the read advance together, one "round" per iteration; in a
-// round every segment applies ITS OWN current minimum rank (segments never interact, so this
-// equals the sequential order segment by segment).  Merging every locally-minimal pair at once
-// would be wrong (SURVEY.md section 7 hard part 5), so only pairs whose rank equals the
-// segment minimum fire.  Pair ranks are cached next to the symbols and only pairs touching a
-// freshly merged token are looked up again (one hash probe sequence each).
+// Passes (all stream-ordered, no host synchronisation):
+//   bpe_segments_kernel<false>  one warp per read: finds the ACGT segments (ballots over 32 classes at a time) and
+//                               counts them per LENGTH BIN (width 8 up to 512 symbols)
+//   bpe_bins_kernel             66 threads: bin -> first slot in the segment list / first work item, longest bins first
+//   bpe_segments_kernel<true>   finds them again, writes the sorted segment list; writes the N / UNK tokens and the
+//                               single-base segments to tmp_tok, holes elsewhere; per-read token counts of those
+//   bpe_merge_kernel            persistent warps take work items from an atomic counter, longest segments first:
+//                               one segment per LANE (2..64 symbols), per 2, 4, 8 LANES (up to 128, 256, 512) or per WARP
+//                               (513..2048).
+//                               Lanes of a warp work on segments of one bin, i.e. of nearly equal length.
+//                               Symbols and cached pair ranks sit in the warp's shared-memory slice, one 32-bit word per
+//                               position (rank << 16 | symbol), interleaved so that the lanes hit different banks.
+//                               A round = min over (rank, position) of the alive pairs, one merge: the right symbol dies
+//                               in place (no compaction), two rule look-ups refresh the ranks of the pairs that touch
+//                               the new token.  No block barrier anywhere; a segment is finished when ITS minimum is
+//                               "no rule".
+//   bpe_merge_giant_kernel      the same code, one warp per CTA with a large slice, for segments over 2048 symbols
+//   scan_counts_kernel, bpe_gather_kernel   token counts -> out_offsets; tokens of tmp_tok -> ids
 #pragma once
 #include "common.cuh"
 
 namespace dtk {
 
-constexpr int BPE_NT = 256;
 constexpr uint32_t BPE_INF = 0xffffu;          // "no rule" rank / also the largest uint16
 constexpr uint32_t SYM_N = 0xffffu, SYM_UNK = 0xfffeu;   // boundary symbols (never merged, never removed)
 constexpr uint64_t HASH_EMPTY = ~0ull;
-constexpr uint32_t SYM_HOLE = 0xfffdu;          // tmp_tok entry that holds no token (the gather kernel drops it)
+constexpr uint32_t SYM_HOLE = 0xfffdu;          // tmp_tok entry that holds no token (the gather kernel drops it);
+                                                //   in the merge workspace: a symbol that was merged into its left neighbour
+
+constexpr int BPE_NB = 66;                      // length bins: 0..63 = 8 lengths each (2..512), 64 = 513..2048, 65 = longer
+constexpr int BPE_MAIN_BINS = 65;               // bins the main merge kernel serves
+constexpr int BPE_SLOT_WORDS = 2048;            // shared-memory words per warp of the main merge kernel
+constexpr int BPE_WARPS = 8;                    // warps per CTA of the main merge kernel
+constexpr int BPE_GIANT_MAX = 49152;            // symbols the giant kernel's slice can hold at most (192 KiB)
+constexpr int BPE_SEG_WARPS = 8;                // warps (= reads in flight) per CTA of the segment finder
+
+struct BpeSeg { uint32_t start, len, read, pad; };   // start: index into cls / tmp_tok of the segment's first symbol
+
+__host__ __device__ __forceinline__ int bpe_bin(uint32_t len) { return len <= 512u ? (int)((len - 1u) >> 3) : (len <= (uint32_t)BPE_SLOT_WORDS ? 64 : 65); }
+// lanes per segment: G lanes share BPE_SLOT_WORDS / (32 / G) positions -- 64 per lane
+__host__ __device__ __forceinline__ int bpe_bin_lanes(int bin) { return bin < 8 ? 1 : (bin < 16 ? 2 : (bin < 32 ? 4 : (bin < 64 ? 8 : 32))); }
+// processing order: longest first (bin 64, 63, ..., 0), the giant bin last (its own kernel)
+__host__ __device__ __forceinline__ int bpe_ord(int bin) { return bin == 65 ? 65 : 64 - bin; }
 
 struct BpeArgs {
-    const uint8_t *cls;            // compact kept classes of all reads (pass A output)
-    const int64_t *koff;           // [n_rec + 1] kept-base CSR offsets (pass A output)
+    const uint8_t *cls;            // compact kept classes of all reads (class pass output)
+    const int64_t *koff;           // [n_rec + 1] kept-base CSR offsets (class pass output)
     int64_t n_rec;
     const uint64_t *table;         // open-addressing hash: (left<<16|right)<<32 | rank
     uint32_t table_mask;
-    int32_t cap;                   // symbols per read the shared-memory workspace can hold
-    uint16_t *tmp_tok;             // per kept base of read r: a token of the segment that started there, or SYM_HOLE
+    uint16_t *tmp_tok;             // per kept base: a token of the segment that started there, or SYM_HOLE
     int32_t *tok_cnt;              // [n_rec] tokens per read
     uint32_t *status;
+    BpeSeg *segs;                  // segment list, sorted by bin in processing order
+    int64_t segs_cap;
+    uint32_t *ctl;                 // control block (zeroed before every call): see the CTL_* offsets
+    int32_t giant_cap;             // symbols the giant kernel's slice holds
 };
+// control block layout (uint32 words)
+constexpr int CTL_CNT = 0;                      // [BPE_NB] segments per bin
+constexpr int CTL_FILL = CTL_CNT + BPE_NB;      // [BPE_NB] fill cursors
+constexpr int CTL_BASE = CTL_FILL + BPE_NB;     // [BPE_NB + 1] by processing order: first slot in segs
+constexpr int CTL_ITEM = CTL_BASE + BPE_NB + 1; // [BPE_NB + 1] by processing order: first work item
+constexpr int CTL_CTR = CTL_ITEM + BPE_NB + 1;  // [2] work-item counters: main, giant
+constexpr int CTL_WORDS = CTL_CTR + 2;
 
 __device__ __forceinline__ uint32_t bpe_hash(uint32_t key) {
     key ^= key >> 15; key *= 0x2c1b3c6du; key ^= key >> 12; key *= 0x297a2d39u; key ^= key >> 15;
@@ -40,204 +79,221 @@ __device__ __forceinline__ uint32_t bpe_hash(uint32_t key) {
 }
 
 __device__ __forceinline__ uint32_t bpe_rank(const BpeArgs &A, uint32_t l, uint32_t r) {
-    if (l >= SYM_UNK || r >= SYM_UNK) return BPE_INF;
     const uint32_t key = (l << 16) | r;
     uint32_t h = bpe_hash(key) & A.table_mask;
     for (;;) {
-        uint64_t s = __ldg(A.table + h);
+        const uint64_t s = __ldg(A.table + h);
         if (s == HASH_EMPTY) return BPE_INF;
         if ((uint32_t)(s >> 32) == key) return (uint32_t)s;
         h = (h + 1) & A.table_mask;
     }
 }
 
-// block-wide exclusive count of a flag (BPE_NT threads), one barrier: ballot + popc inside the warp, the warp totals
-// through shared memory.  Consecutive calls alternate between the two halves of warp_tmp (pp), so a warp still
-// reading one half never meets the writes of the next call.
-__device__ __forceinline__ int bpe_exscan(bool f, int (*warp_tmp)[BPE_NT / 32], int &pp, int &total) {
-    static_assert((BPE_NT / 32) % 4 == 0, "warp totals are read four at a time");
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const uint32_t b = __ballot_sync(0xffffffffu, f);
-    if (lane == 0) warp_tmp[pp][warp] = __popc(b);
-    __syncthreads();
-    int woff = 0, tot = 0;
-#pragma unroll
-    for (int q = 0; q < BPE_NT / 128; ++q) {
-        const int4 t = *reinterpret_cast<const int4 *>(&warp_tmp[pp][4 * q]);
-        const int v[4] = {t.x, t.y, t.z, t.w};
-#pragma unroll
-        for (int j = 0; j < 4; ++j) { if (4 * q + j < warp) woff += v[j]; tot += v[j]; }
-    }
-    pp ^= 1;
-    total = tot;
-    return woff + __popc(b & ((1u << lane) - 1u));
-}
-
-// minimum of rank rk into the 16-bit slot of segment sg (two slots per 32-bit word, CAS on the word)
-__device__ __forceinline__ void bpe_seg_min(uint16_t *segmin, uint32_t sg, uint32_t rk) {
-    uint32_t *w = reinterpret_cast<uint32_t *>(segmin) + (sg >> 1);
-    uint32_t old = *w;
-    for (;;) {
-        const uint32_t half = (sg & 1) ? (old >> 16) : (old & 0xffffu);
-        if (half <= rk) break;
-        const uint32_t neu = (sg & 1) ? ((old & 0xffffu) | (rk << 16)) : ((old & 0xffff0000u) | rk);
-        const uint32_t got = atomicCAS(w, old, neu);
-        if (got == old) break;
-        old = got;
-    }
-}
-
-// ranks of one warp's 32 consecutive symbols into the per-segment minima: segments are contiguous, so a segmented
-// min-scan over the warp leaves each run's minimum in its last lane, which alone touches shared memory
-__device__ __forceinline__ bool bpe_warp_seg_min(uint16_t *segmin, uint32_t sg, uint32_t rk, bool valid) {
+// ---- segment finder ----------------------------------------------------------------------------------------
+// One warp per read, 32 classes per step.  FILL = false: counts the segments of 2 or more symbols per length bin.
+// FILL = true: writes their records into the bin-sorted list, the tokens that need no merging (N, UNK, single bases) to
+// tmp_tok with holes everywhere else, and the number of those tokens to tok_cnt.
+template <bool FILL>
+__global__ void __launch_bounds__(BPE_SEG_WARPS * 32) bpe_segments_kernel(const __grid_constant__ BpeArgs A) {
     constexpr uint32_t FULL = 0xffffffffu;
-    const int lane = threadIdx.x & 31;
-    if (!valid) { sg = 0xffffffffu; rk = BPE_INF; }
-    uint32_t v = rk;
-#pragma unroll
-    for (int d = 1; d < 32; d <<= 1) {
-        const uint32_t t = __shfl_up_sync(FULL, v, d), st = __shfl_up_sync(FULL, sg, d);
-        if (lane >= d && st == sg) v = min(v, t);
+    __shared__ uint32_t hist[BPE_NB];           // segments of this CTA's reads per bin, then the fill cursor inside the CTA's range
+    __shared__ uint32_t first[BPE_NB];          // FILL: first slot of the CTA's range in each bin
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int64_t r = (int64_t)blockIdx.x * BPE_SEG_WARPS + warp;
+    for (int i = tid; i < BPE_NB; i += blockDim.x) hist[i] = 0u;
+    __syncthreads();
+    const bool have = r < A.n_rec;
+    const int64_t k0 = have ? A.koff[r] : 0;
+    const int n = have ? (int)(A.koff[r + 1] - k0) : 0;
+
+    // sweep(emit): calls emit(start, len) once per segment (start relative to the read), from one lane
+    auto sweep = [&](auto &&emit) {
+        int open = -1;                          // start of the segment still open at the end of the previous step
+        for (int base = 0; base < n; base += 32) {
+            const int i = base + lane;
+            const uint32_t c = i < n ? A.cls[k0 + i] : 255u;
+            const uint32_t bm = __ballot_sync(FULL, c >= CLS_N);          // boundaries (positions past the end count as one)
+            const bool prevb = lane ? ((bm >> (lane - 1)) & 1u) : (open < 0);
+            const bool st = c < CLS_N && prevb;                           // a segment starts here
+            if (open >= 0 && bm && lane == 0) emit(open, base + __ffs(bm) - 1 - open);
+            const uint32_t above = lane == 31 ? 0u : (bm & (FULL << (lane + 1)));
+            if (st && above) emit(i, base + __ffs(above) - 1 - i);
+            if (bm == 0u) { if (open < 0) open = base; }
+            else { const int lastb = 31 - __clz(bm); open = lastb < 31 ? base + lastb + 1 : -1; }
+        }
+        if (open >= 0 && lane == 0) emit(open, n - open);                 // (n is a multiple of 32 and the read ends open)
+    };
+
+    sweep([&](int, int len) { if (len >= 2 && len <= A.giant_cap) atomicAdd(&hist[bpe_bin((uint32_t)len)], 1u); });
+    __syncthreads();
+    if (!FILL) {
+        for (int i = tid; i < BPE_NB; i += blockDim.x) if (hist[i]) atomicAdd(&A.ctl[CTL_CNT + i], hist[i]);
+        return;
     }
-    const uint32_t nsg = __shfl_down_sync(FULL, sg, 1);
-    const bool last = lane == 31 || nsg != sg;
-    if (valid && last && v != BPE_INF) bpe_seg_min(segmin, sg, v);
-    return __any_sync(FULL, valid && rk != BPE_INF);
+    for (int i = tid; i < BPE_NB; i += blockDim.x) {
+        first[i] = hist[i] ? A.ctl[CTL_BASE + bpe_ord(i)] + atomicAdd(&A.ctl[CTL_FILL + i], hist[i]) : 0u;
+        hist[i] = 0u;
+    }
+    __syncthreads();
+    // tokens that need no merging, holes elsewhere
+    int direct = 0;
+    for (int base = 0; base < n; base += 32) {
+        const int i = base + lane;
+        if (i < n) {
+            const uint32_t c = A.cls[k0 + i];
+            A.tmp_tok[k0 + i] = (uint16_t)(c < CLS_N ? SYM_HOLE : (c == CLS_N ? SYM_N : SYM_UNK));
+            direct += c >= CLS_N;
+        }
+    }
+    __syncwarp();
+    sweep([&](int start, int len) {
+        if (len == 1) { A.tmp_tok[k0 + start] = (uint16_t)A.cls[k0 + start]; ++direct; return; }
+        const int bin = bpe_bin((uint32_t)len);
+        if (len > A.giant_cap) { A.status[0] = 1u; return; }               // does not fit any workspace: reported, no tokens
+        const uint32_t slot = first[bin] + atomicAdd(&hist[bin], 1u);
+        if ((int64_t)slot < A.segs_cap) A.segs[slot] = BpeSeg{(uint32_t)(k0 + start), (uint32_t)len, (uint32_t)r, 0u};
+        else A.status[0] = 1u;
+    });
+    direct = __reduce_add_sync(FULL, direct);
+    if (have && lane == 0) A.tok_cnt[r] = direct;
 }
 
-// dynamic shared memory layout: sym[2][cap] rnk[2][cap] seg[2][cap] src[cap] segmin[2][cap+2] origin[cap]
-// segstart[cap], all uint16.  A segment none of whose pairs has a rule any more is finished: the next compaction pass
-// writes its tokens to tmp_tok at the segment's own place in the read (the rest of its span stays SYM_HOLE) and drops
-// it from the working sequence, so late rounds only touch the few long segments that are still merging.
-// One round = compaction pass (one barrier per chunk of BPE_NT symbols) -> barrier -> rank pass, which also collects
-// the next round's per-segment minima into the other segmin buffer -> barrier.
-__global__ void __launch_bounds__(BPE_NT) bpe_reads_kernel(const __grid_constant__ BpeArgs A) {
-    extern __shared__ __align__(16) uint16_t sh[];
-    __shared__ __align__(16) int warp_tmp[2][BPE_NT / 32];
-    const int cap = A.cap, tid = threadIdx.x;
-    uint16_t *symb[2] = {sh, sh + cap};
-    uint16_t *rnkb[2] = {sh + 2 * cap, sh + 3 * cap};
-    uint16_t *segb[2] = {sh + 4 * cap, sh + 5 * cap};
-    uint16_t *src = sh + 6 * cap;
-    uint16_t *sminb[2] = {sh + 7 * cap, sh + 8 * cap + 2};
-    uint16_t *origin = sh + 9 * cap + 4;       // [cap] position in the read of each segment's first symbol
-    uint16_t *segstart = sh + 10 * cap + 4;    // [cap] index in the current sequence of each segment's first symbol
-    __shared__ int s_cnt;
-    int pp = 0;
+// bin counts -> list slots and work items, in processing order
+__global__ void __launch_bounds__(128) bpe_bins_kernel(const __grid_constant__ BpeArgs A) {
+    __shared__ uint32_t cnt[BPE_NB], items[BPE_NB];
+    const int o = threadIdx.x;                  // processing-order index
+    if (o < BPE_NB) {
+        const int bin = o == 65 ? 65 : 64 - o;
+        const uint32_t c = A.ctl[CTL_CNT + bin];
+        cnt[o] = c;
+        const uint32_t per = 32u / (uint32_t)bpe_bin_lanes(bin);          // segments per work item
+        items[o] = (c + per - 1u) / per;
+    }
+    __syncthreads();
+    if (o == 0) {
+        uint32_t s = 0, t = 0;
+        for (int i = 0; i < BPE_NB; ++i) {
+            A.ctl[CTL_BASE + i] = s; A.ctl[CTL_ITEM + i] = t;
+            s += cnt[i]; t += items[i];
+        }
+        A.ctl[CTL_BASE + BPE_NB] = s; A.ctl[CTL_ITEM + BPE_NB] = t;
+    }
+}
 
-    for (int64_t r = blockIdx.x; r < A.n_rec; r += gridDim.x) {
-        const int64_t k0 = A.koff[r];
-        const int64_t n64 = A.koff[r + 1] - k0;
-        __syncthreads();
-        if (n64 > cap) {                      // read does not fit the workspace: report, emit nothing
-            if (tid == 0) { A.status[0] = 1u; A.tok_cnt[r] = 0; }
-            continue;
+// ---- the merge loop: G lanes per segment, 32 / G segments per warp ------------------------------------------------
+// slice: the warp's shared-memory words; position i of the warp's group q sits at slice[i * (32 / G) + q].
+template <int G>
+__device__ __forceinline__ void bpe_merge_item(const BpeArgs &A, uint32_t *slice, uint32_t seg_lo, uint32_t seg_hi, int lane) {
+    constexpr uint32_t FULL = 0xffffffffu;
+    constexpr int NG = 32 / G;
+    const int q = lane / G, g = lane % G;
+    const uint32_t si = seg_lo + (uint32_t)q;
+    const bool have = si < seg_hi;
+    BpeSeg sg = BpeSeg{0u, 0u, 0u, 0u};
+    if (have) sg = A.segs[si];
+    const int L = (int)sg.len;
+    uint32_t *w = slice + q;
+    // symbols, then the rank of every adjacent pair
+    for (int i = g; i < L; i += G) w[i * NG] = (BPE_INF << 16) | (uint32_t)A.cls[sg.start + i];
+    if (G > 1) __syncwarp();
+    for (int i = g; i + 1 < L; i += G) {
+        const uint32_t s0 = w[i * NG] & 0xffffu, s1 = w[(i + 1) * NG] & 0xffffu;
+        w[i * NG] = (bpe_rank(A, s0, s1) << 16) | s0;
+    }
+    if (G > 1) __syncwarp();
+    bool done = L < 2;
+    for (;;) {
+        // lowest (rank, position) over the segment's alive pairs
+        uint32_t key = 0xffffffffu;
+        if (!done) {
+            int i = g;
+#pragma unroll 4
+            for (; i < L; i += G) key = min(key, (w[i * NG] & 0xffff0000u) | (uint32_t)i);
         }
-        int n = (int)n64, cur = 0, ms = 0;
-        // ---- load symbols, segment ids (a boundary symbol forms its own segment) --------
-        // seg id = number of "segment starts" at or before i, minus 1; a start is i == 0, a boundary,
-        // or the position right after a boundary.
-        for (int i = tid; i < n; i += BPE_NT) {
-            const uint32_t c = A.cls[k0 + i];
-            symb[0][i] = (uint16_t)(c < CLS_N ? c : (c == CLS_N ? SYM_N : SYM_UNK));
-        }
-        for (int i = tid; i <= n; i += BPE_NT) sminb[0][i] = (uint16_t)BPE_INF;     // at most n segments
-        for (int i = tid; i < n; i += BPE_NT) A.tmp_tok[k0 + i] = (uint16_t)SYM_HOLE;
-        if (tid == 0) s_cnt = 0;
-        __syncthreads();
-        int seg_base = 0;
-        for (int base = 0; base < n; base += BPE_NT) {       // chunked so the scan carries across chunks
-            int i = base + tid;
-            int start = 0;
-            if (i < n) {
-                bool bd = symb[0][i] >= SYM_UNK;
-                bool pb = (i > 0) && symb[0][i - 1] >= SYM_UNK;
-                start = (i == 0 || bd || pb) ? 1 : 0;
+#pragma unroll
+        for (int d = G >> 1; d > 0; d >>= 1) key = min(key, __shfl_xor_sync(FULL, key, d));
+        if ((key >> 16) == BPE_INF) done = true;
+        if (__all_sync(FULL, done)) break;
+        if (!done) {
+            const uint32_t m = key >> 16;
+            const int bi = (int)(key & 0xffffu);
+            int j = bi + 1;                                   // the pair's right symbol: the next alive one (it exists)
+            while ((w[j * NG] & 0xffffu) == SYM_HOLE) ++j;
+            int jn = j + 1;                                   // the alive symbol behind it, if any
+            while (jn < L && (w[jn * NG] & 0xffffu) == SYM_HOLE) ++jn;
+            int p = bi - 1;                                   // the alive symbol in front, if any
+            while (p >= 0 && (w[p * NG] & 0xffffu) == SYM_HOLE) --p;
+            const uint32_t ns = 4u + m;
+            if (g == 0) {
+                const uint32_t r1 = jn < L ? bpe_rank(A, ns, w[jn * NG] & 0xffffu) : BPE_INF;
+                w[bi * NG] = (r1 << 16) | ns;
+                w[j * NG] = (BPE_INF << 16) | SYM_HOLE;
             }
-            int tot;
-            int ex = bpe_exscan(start != 0, warp_tmp, pp, tot);
-            uint32_t sg = 0, rk = BPE_INF;
-            if (i < n) {
-                sg = (uint32_t)(seg_base + ex + start - 1);
-                segb[0][i] = (uint16_t)sg;
-                if (start) { origin[sg] = (uint16_t)i; segstart[sg] = (uint16_t)i; }
-                rk = (i + 1 < n) ? bpe_rank(A, symb[0][i], symb[0][i + 1]) : BPE_INF;
-                rnkb[0][i] = (uint16_t)rk;
+            if (g == (G > 1 ? 1 : 0) && p >= 0) {
+                const uint32_t sp = w[p * NG] & 0xffffu;
+                w[p * NG] = (bpe_rank(A, sp, ns) << 16) | sp;
             }
-            bpe_warp_seg_min(sminb[0], sg, rk, i < n);
-            seg_base += tot;
         }
-        __syncthreads();
+        if (G > 1) __syncwarp();
+    }
+    // tokens of the segment, in order, at the segment's own place
+    if (have && g == 0) {
+        int cnt = 0;
+        for (int i = 0; i < L; ++i) {
+            const uint32_t s = w[i * NG] & 0xffffu;
+            if (s != SYM_HOLE) A.tmp_tok[sg.start + cnt++] = (uint16_t)s;
+        }
+        atomicAdd(&A.tok_cnt[sg.read], cnt);
+    }
+}
 
-        // ---- rounds ----------------------------------------------------------------------
-        while (n > 0) {
-            uint16_t *sym = symb[cur], *rnk = rnkb[cur], *seg = segb[cur], *segmin = sminb[ms];
-            uint16_t *sym2 = symb[cur ^ 1], *rnk2 = rnkb[cur ^ 1], *seg2 = segb[cur ^ 1], *smin2 = sminb[ms ^ 1];
-            // the other minima buffer gets ready for the rank pass of this round
-            for (int i = tid; i <= seg_base; i += BPE_NT) smin2[i] = (uint16_t)BPE_INF;
-            // flags, run parity, compaction
-            int carry = 0;
-            for (int base = 0; base < n; base += BPE_NT) {
-                int i = base + tid;
-                bool keep = false, merge = false;
-                {
-                    auto fires = [&](int j) -> bool {            // pair (j, j+1) is selected (before overlap rule)
-                        uint32_t rk = rnk[j];
-                        return rk != BPE_INF && rk == segmin[seg[j]];
-                    };
-                    auto merges = [&](int j) -> bool {           // left to right, non-overlapping (Q11)
-                        if (!fires(j)) return false;
-                        int c = 0;
-                        while (j - 1 - c >= 0 && fires(j - 1 - c)) ++c;
-                        return (c & 1) == 0;
-                    };
-                    // one look at the symbol's own pair; the run of selected pairs in front of it comes from the warp's
-                    // ballot, and only a run that reaches the warp's first lane is followed back through shared memory
-                    const int ln = tid & 31;
-                    // a finished segment leaves: its tokens go to their place in the read
-                    const uint32_t sgi = i < n ? (uint32_t)seg[i] : 0u;
-                    const bool fin = i < n && segmin[sgi] == BPE_INF;
-                    if (fin) A.tmp_tok[k0 + origin[sgi] + (i - (int)segstart[sgi])] = sym[i];
-                    const uint32_t fb = __ballot_sync(0xffffffffu, fin);
-                    if (ln == 0 && fb) atomicAdd(&s_cnt, __popc(fb));
-                    const bool f = i < n && !fin && fires(i);
-                    const uint32_t Fw = __ballot_sync(0xffffffffu, f);
-                    int c = ln ? __clz(~(Fw << (32 - ln))) : 0;  // selected pairs directly in front, inside the warp
-                    if (c > ln) c = ln;
-                    if (f && c == ln) { int j = i - ln - 1; while (j >= 0 && fires(j)) { ++c; --j; } }
-                    merge = f && (c & 1) == 0;
-                    const bool pm = __shfl_up_sync(0xffffffffu, merge, 1);
-                    if (i < n && !fin) keep = !(ln ? pm : (i > 0 && merges(i - 1)));
-                }
-                int tot;
-                int w = carry + bpe_exscan(keep, warp_tmp, pp, tot);
-                if (keep) {
-                    sym2[w] = merge ? (uint16_t)(4u + rnk[i]) : sym[i];
-                    seg2[w] = seg[i];
-                    if (i == 0 || seg[i - 1] != seg[i]) segstart[seg[i]] = (uint16_t)w;   // first symbol of its segment
-                    src[w] = (uint16_t)(merge ? 0xffffu : i);    // 0xffff: freshly merged token
-                }
-                carry += tot;
-            }
-            __syncthreads();
-            const int n2 = carry;
-            for (int base = 0; base < n2; base += BPE_NT) {
-                const int w = base + tid;
-                uint32_t rk = BPE_INF, sg = 0;
-                if (w < n2) {
-                    if (w + 1 < n2 && seg2[w] == seg2[w + 1]) {      // neighbours of different segments never pair
-                        if (src[w] == 0xffffu || src[w + 1] == 0xffffu) rk = bpe_rank(A, sym2[w], sym2[w + 1]);
-                        else rk = rnk[src[w]];
-                    }
-                    rnk2[w] = (uint16_t)rk;
-                    sg = seg2[w];
-                }
-                bpe_warp_seg_min(smin2, sg, rk, w < n2);
-            }
-            n = n2; cur ^= 1; ms ^= 1;
-            __syncthreads();
-        }
-        if (tid == 0) A.tok_cnt[r] = s_cnt;     // every token has been written by the pass that retired its segment
+__global__ void __launch_bounds__(BPE_WARPS * 32) bpe_merge_kernel(const __grid_constant__ BpeArgs A) {
+    extern __shared__ __align__(16) uint32_t bpe_smem[];
+    constexpr uint32_t FULL = 0xffffffffu;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    uint32_t *slice = bpe_smem + warp * BPE_SLOT_WORDS;
+    // work-item table (processing order), three entries per lane
+    uint32_t ib[3];
+#pragma unroll
+    for (int x = 0; x < 3; ++x) { const int o = lane + 32 * x; ib[x] = o <= BPE_MAIN_BINS ? A.ctl[CTL_ITEM + o] : 0xffffffffu; }
+    const uint32_t n_items = A.ctl[CTL_ITEM + BPE_MAIN_BINS];
+    for (;;) {
+        uint32_t t = 0;
+        if (lane == 0) t = atomicAdd(&A.ctl[CTL_CTR], 1u);
+        t = __shfl_sync(FULL, t, 0);
+        if (t >= n_items) break;
+        // o = last processing-order index whose first item is <= t
+        int o = 0;
+#pragma unroll
+        for (int x = 0; x < 3; ++x) o += __popc(__ballot_sync(FULL, ib[x] <= t));
+        o -= 1;
+        // (empty bins share their first item with the next one: the last such index is the bin that owns item t)
+        const int bin = 64 - o;
+        const int G = bpe_bin_lanes(bin);
+        const uint32_t lo = A.ctl[CTL_BASE + o] + (t - A.ctl[CTL_ITEM + o]) * (uint32_t)(32 / G);
+        const uint32_t hi = A.ctl[CTL_BASE + o + 1];
+        if (G == 1) bpe_merge_item<1>(A, slice, lo, hi, lane);
+        else if (G == 2) bpe_merge_item<2>(A, slice, lo, hi, lane);
+        else if (G == 4) bpe_merge_item<4>(A, slice, lo, hi, lane);
+        else if (G == 8) bpe_merge_item<8>(A, slice, lo, hi, lane);
+        else bpe_merge_item<32>(A, slice, lo, hi, lane);
+        __syncwarp();
+    }
+}
+
+// segments over BPE_SLOT_WORDS symbols: one warp per CTA, the whole dynamic shared memory is its slice
+__global__ void __launch_bounds__(32) bpe_merge_giant_kernel(const __grid_constant__ BpeArgs A) {
+    extern __shared__ __align__(16) uint32_t bpe_smem[];
+    constexpr uint32_t FULL = 0xffffffffu;
+    const int lane = threadIdx.x;
+    const uint32_t lo = A.ctl[CTL_BASE + 65], hi = A.ctl[CTL_BASE + 66];
+    for (;;) {
+        uint32_t t = 0;
+        if (lane == 0) t = atomicAdd(&A.ctl[CTL_CTR + 1], 1u);
+        t = __shfl_sync(FULL, t, 0);
+        if (lo + t >= hi) break;
+        bpe_merge_item<32>(A, bpe_smem, lo + t, hi, lane);
+        __syncwarp();
     }
 }
 
@@ -285,7 +341,7 @@ __global__ void __launch_bounds__(256) bpe_gather_kernel(const uint16_t *tmp_tok
             const uint32_t s = i < n ? (uint32_t)tmp_tok[k0 + i] : SYM_HOLE;
             const uint32_t vm = __ballot_sync(FULL, s != SYM_HOLE);
             const int64_t at = o + __popc(vm & ((1u << lane) - 1u));
-            if (s != SYM_HOLE && at < o_end) {               // (a read that did not fit the workspace has no tokens)
+            if (s != SYM_HOLE && at < o_end) {               // (a segment that did not fit the workspace has no tokens)
                 const int32_t id = s == SYM_N ? n_id : (s == SYM_UNK ? unk_id : (int32_t)(base_id + s));
                 if (at < ids_cap) ids[at] = (IdT)id; else status[0] = 1u;
             }

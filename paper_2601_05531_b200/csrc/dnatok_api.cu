@@ -41,6 +41,8 @@ struct EncCtx {
     uint8_t *cls = nullptr;  int64_t cls_cap = 0;
     uint16_t *tmp_tok = nullptr;
     int64_t *koff = nullptr; int32_t *tok_cnt = nullptr; int64_t rec_cap = 0;
+    BpeSeg *segs = nullptr; int64_t segs_cap = 0;   // bin-sorted ACGT segments of 2 or more symbols
+    uint32_t *bpe_ctl = nullptr;                    // bin counts, list slots, work items, work-item counters
 };
 
 struct StreamSlot {
@@ -127,7 +129,7 @@ int ctx_init(dnatok_t *h, EncCtx &c) {
 void ctx_free(EncCtx &c) {
     cudaFree(c.descs); cudaFree(c.gdescs); cudaFree(c.ls); cudaFree(c.first_rec); cudaFree(c.rec_k); cudaFree(c.ticket); cudaFreeHost(c.h_status);
     cudaFree(c.prof);
-    cudaFree(c.cls); cudaFree(c.tmp_tok); cudaFree(c.koff); cudaFree(c.tok_cnt);
+    cudaFree(c.cls); cudaFree(c.tmp_tok); cudaFree(c.koff); cudaFree(c.tok_cnt); cudaFree(c.segs); cudaFree(c.bpe_ctl);
     c = EncCtx();
 }
 
@@ -261,6 +263,7 @@ int ctx_reserve_bpe(dnatok_t *h, EncCtx &c, int64_t n_bytes, int64_t n_rec, cuda
         CU(cudaMallocAsync((void **)&c.tmp_tok, (size_t)cap * sizeof(uint16_t), st));
         c.cls_cap = cap;
     }
+    if (!c.bpe_ctl) CU(cudaMallocAsync((void **)&c.bpe_ctl, CTL_WORDS * sizeof(uint32_t), st));
     if (n_rec + 1 > c.rec_cap) {
         int64_t cap = n_rec + n_rec / 8 + 256;
         if (c.koff) CU(cudaFreeAsync(c.koff, st));
@@ -273,7 +276,6 @@ int ctx_reserve_bpe(dnatok_t *h, EncCtx &c, int64_t n_bytes, int64_t n_rec, cuda
     return DNATOK_OK;
 }
 
-size_t bpe_smem_bytes(int cap) { return (size_t)(11 * cap + 8) * sizeof(uint16_t); }
 
 int encode_on(dnatok_t *h, EncCtx &c, const uint8_t *d_bytes, int64_t n_bytes, const int64_t *d_rec_off,
               int64_t n_rec, int64_t off_bias, void *d_ids, int64_t ids_cap, int64_t *d_out_off, cudaStream_t st) {
@@ -292,14 +294,35 @@ int encode_on(dnatok_t *h, EncCtx &c, const uint8_t *d_bytes, int64_t n_bytes, c
     rc = launch_tiles<uint8_t>(h, c, pa, d_bytes, n_bytes, d_rec_off, n_rec, off_bias, c.cls, c.cls_cap, c.koff, st);
     if (rc) return rc;
     if (n_rec > 0) {
+        if (n_bytes >= (1ll << 32)) return fail(h, DNATOK_EINVAL, "BPE: one call encodes less than 4 GiB (split the input)");
+        // a segment of two or more symbols is followed by a boundary symbol or by the end of its read
+        if (c.segs_cap < n_bytes / 3 + n_rec + 16) {
+            if (c.segs) CU(cudaFreeAsync(c.segs, st));
+            c.segs = nullptr; c.segs_cap = 0;
+            const int64_t scap = n_bytes / 3 + n_rec + n_rec / 8 + 16;
+            CU(cudaMallocAsync((void **)&c.segs, (size_t)scap * sizeof(BpeSeg), st));
+            c.segs_cap = scap;
+        }
         BpeArgs b;
         b.cls = c.cls; b.koff = c.koff; b.n_rec = n_rec; b.table = h->d_table; b.table_mask = h->table_mask;
-        b.cap = h->bpe_cap; b.tmp_tok = c.tmp_tok; b.tok_cnt = c.tok_cnt; b.status = c.d_status;
-        int grid = (int)std::min<int64_t>(n_rec, (int64_t)h->sm_count * h->bpe_ctas_per_sm);
+        b.tmp_tok = c.tmp_tok; b.tok_cnt = c.tok_cnt; b.status = c.d_status;
+        b.segs = c.segs; b.segs_cap = c.segs_cap; b.ctl = c.bpe_ctl; b.giant_cap = h->bpe_cap;
+        CU(cudaMemsetAsync(c.bpe_ctl, 0, CTL_WORDS * sizeof(uint32_t), st));
+        const unsigned nb_seg = (unsigned)((n_rec + BPE_SEG_WARPS - 1) / BPE_SEG_WARPS);
+        bpe_segments_kernel<false><<<nb_seg, BPE_SEG_WARPS * 32, 0, st>>>(b);
+        bpe_bins_kernel<<<1, 128, 0, st>>>(b);
+        bpe_segments_kernel<true><<<nb_seg, BPE_SEG_WARPS * 32, 0, st>>>(b);
+        int grid = h->sm_count * h->bpe_ctas_per_sm;
         if (h->grid_cap > 0) grid = std::min(grid, h->grid_cap);
-        bpe_reads_kernel<<<grid, BPE_NT, bpe_smem_bytes(h->bpe_cap), st>>>(b);
+        bpe_merge_kernel<<<grid, BPE_WARPS * 32, BPE_WARPS * BPE_SLOT_WORDS * sizeof(uint32_t), st>>>(b);
+        if (h->bpe_cap > BPE_SLOT_WORDS) {
+            int gg = h->sm_count;
+            if (h->grid_cap > 0) gg = std::min(gg, h->grid_cap);
+            bpe_merge_giant_kernel<<<gg, 32, (size_t)h->bpe_cap * sizeof(uint32_t), st>>>(b);
+            h->launches += 1;
+        }
         CU(cudaGetLastError());
-        h->launches += 1;
+        h->launches += 4;
     }
     scan_counts_kernel<<<1, 1024, 0, st>>>(c.tok_cnt, n_rec, d_out_off);
     CU(cudaGetLastError());
@@ -484,13 +507,17 @@ int dnatok_create(const dnatok_config *cfg_in, int device, dnatok_t **out) {
         if (cudaMalloc(&h->d_table, table.size() * sizeof(uint64_t)) != cudaSuccess) return bail(DNATOK_ENOMEM);
         if (cudaMemcpy(h->d_table, table.data(), table.size() * sizeof(uint64_t), cudaMemcpyHostToDevice) != cudaSuccess)
             return bail(DNATOK_ECUDA);
-        // per-read workspace: the smaller it is, the more reads are in flight per SM, and that is what sets the rate
-        int cap = (int)std::min<int64_t>(8192, std::max<int64_t>(256, (cfg.max_record_bytes + 63) & ~(int64_t)63));
+        // longest ACGT segment (run between N / UNK bytes) the merge kernels hold: up to 2048 symbols in the main kernel's
+        // per-warp slice, up to BPE_GIANT_MAX in the giant kernel's (one warp per SM); longer ones are ECAPACITY
+        int cap = (int)std::min<int64_t>(BPE_GIANT_MAX, std::max<int64_t>(BPE_SLOT_WORDS, (cfg.max_record_bytes + 63) & ~(int64_t)63));
         h->bpe_cap = cap;
-        if (cudaFuncSetAttribute(bpe_reads_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                 (int)bpe_smem_bytes(cap)) != cudaSuccess) return bail(DNATOK_ECUDA);
+        const int main_smem = BPE_WARPS * BPE_SLOT_WORDS * (int)sizeof(uint32_t);
+        if (cudaFuncSetAttribute(bpe_merge_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, main_smem) != cudaSuccess)
+            return bail(DNATOK_ECUDA);
+        if (cap > BPE_SLOT_WORDS && cudaFuncSetAttribute(bpe_merge_giant_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                               cap * (int)sizeof(uint32_t)) != cudaSuccess) return bail(DNATOK_ECUDA);
         int nb = 0;
-        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, bpe_reads_kernel, BPE_NT, bpe_smem_bytes(cap));
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, bpe_merge_kernel, BPE_WARPS * 32, main_smem);
         h->bpe_ctas_per_sm = std::max(nb, 1);
     }
     {

@@ -317,24 +317,45 @@ def test_bpe_homopolymer_runs_and_fasta_layout():
     check(data, [0, len(data)], mode="bpe", merges=merges, max_record_bytes=2048)
 
 
-def test_bpe_segment_lengths_around_the_lane_slot():
-    """segments of 383 / 384 / 385 / 1 bases: the lane-per-segment kernel holds at most 384 symbols per lane, longer
-    segments send their read to the block-per-read kernel; reads of both kinds sit side by side"""
+def test_bpe_segment_lengths_around_the_group_sizes():
+    """segments on both sides of every length class of the merge kernel (one segment per lane up to 64 symbols, per 2 / 4 /
+    8 lanes up to 128 / 256 / 512, per warp up to 2048, the giant kernel beyond), side by side in the same reads, and
+    lengths on both sides of a 32-class step of the segment finder"""
     rng = random.Random(7)
     merges = dnagen.merge_table(seed=3, n_merges=200, corpus_bases=8192)
     seg = lambda n: "".join(rng.choice("ACGT") for _ in range(n))
-    recs = [seg(383) + "N" + seg(384) + "N" + seg(1), seg(385) + "NN" + seg(2) + "N", seg(384), "N" + seg(384) + "R" + seg(50),
-            seg(1200), seg(40) + "N" + seg(700) + "N" + seg(40), "", "N", seg(1)]
+    recs = [seg(63) + "N" + seg(64) + "N" + seg(65) + "N" + seg(1), seg(127) + "NN" + seg(128) + "N" + seg(129) + "N",
+            seg(255) + "R" + seg(256) + "N" + seg(257), seg(511) + "N" + seg(512) + "N" + seg(513), seg(2047) + "N" + seg(2), seg(2048),
+            "N" + seg(2049) + "R" + seg(50), seg(5000), seg(31) + "N" + seg(32) + "N" + seg(33) + "N" + seg(31), seg(32), seg(64) + "N",
+            "", "N", seg(1), seg(2), "NN", seg(8) + "N" + seg(9) + "N" + seg(16) + "N" + seg(17)]
     data = np.frombuffer("".join(recs).encode(), dtype=np.uint8)
     offs = np.cumsum([0] + [len(r) for r in recs])
-    check(data, offs, mode="bpe", merges=merges, max_record_bytes=2048)
+    check(data, offs, mode="bpe", merges=merges, max_record_bytes=8192)
 
 
-def test_bpe_read_longer_than_workspace_reports_capacity():
+def test_bpe_many_segments_of_every_bin():
+    """a few thousand segments of every length from 1 to 520 (every 8-wide length bin, work items that are not full) and
+    a table whose rules keep firing on random ACGT"""
+    rng = random.Random(11)
+    merges = dnagen.merge_table(seed=5, n_merges=1500, corpus_bases=65536)
+    recs, cur = [], []
+    for n in list(range(1, 521)) * 3:
+        cur.append("".join(rng.choice("ACGT") for _ in range(n)))
+        if len(cur) == 7:
+            recs.append("N".join(cur)); cur = []
+    recs.append("N".join(cur))
+    data = np.frombuffer("".join(recs).encode(), dtype=np.uint8)
+    offs = np.cumsum([0] + [len(r) for r in recs])
+    check(data, offs, mode="bpe", merges=merges, max_record_bytes=8192)
+
+
+def test_bpe_segment_longer_than_workspace_reports_capacity():
+    """the merge kernels hold ACGT segments of up to max(2048, max_record_bytes) symbols (at most 49152); a longer run between
+    two N / UNK bytes is reported as ECAPACITY"""
     merges = np.array([[0, 1]], dtype=np.int32)
     tok = dn.DNATok(mode="bpe", merges=merges, max_record_bytes=256)
-    d = torch.from_numpy(np.frombuffer(b"AC" * 400, dtype=np.uint8).copy()).cuda()
-    o = torch.tensor([0, 800], dtype=torch.int64, device="cuda")
+    d = torch.from_numpy(np.frombuffer(b"AC" * 1500, dtype=np.uint8).copy()).cuda()
+    o = torch.tensor([0, 3000], dtype=torch.int64, device="cuda")
     tok.encode(d, o)
     with pytest.raises(dn.DNATokError) as e:
         tok.check()
