@@ -63,6 +63,7 @@ struct BpeArgs {
     BpeSeg *segs;                  // segment list, sorted by bin in processing order
     int64_t segs_cap;
     uint32_t *ctl;                 // control block (zeroed before every call): see the CTL_* offsets
+    uint32_t *cta_hist;            // [CTAs of the segment finder][BPE_NB] segments per bin of each CTA's reads (count pass -> fill pass)
     int32_t giant_cap;             // symbols the giant kernel's slice holds
 };
 // control block layout (uint32 words)
@@ -106,12 +107,21 @@ __global__ void __launch_bounds__(BPE_SEG_WARPS * 32) bpe_segments_kernel(const 
     const int64_t k0 = have ? A.koff[r] : 0;
     const int n = have ? (int)(A.koff[r + 1] - k0) : 0;
 
-    // sweep(emit): calls emit(start, len) once per segment (start relative to the read), from one lane
+    // sweep(emit): calls emit(start, len) once per segment (start relative to the read), from one lane.  With FILL it also
+    // writes the tokens that need no merging (N, UNK) and holes everywhere else, before the emits of the same step.
+    int direct = 0;
     auto sweep = [&](auto &&emit) {
         int open = -1;                          // start of the segment still open at the end of the previous step
         for (int base = 0; base < n; base += 32) {
             const int i = base + lane;
             const uint32_t c = i < n ? A.cls[k0 + i] : 255u;
+            if (FILL) {
+                if (i < n) {
+                    A.tmp_tok[k0 + i] = (uint16_t)(c < CLS_N ? SYM_HOLE : (c == CLS_N ? SYM_N : SYM_UNK));
+                    direct += c >= CLS_N;
+                }
+                __syncwarp();
+            }
             const uint32_t bm = __ballot_sync(FULL, c >= CLS_N);          // boundaries (positions past the end count as one)
             const bool prevb = lane ? ((bm >> (lane - 1)) & 1u) : (open < 0);
             const bool st = c < CLS_N && prevb;                           // a segment starts here
@@ -124,28 +134,22 @@ __global__ void __launch_bounds__(BPE_SEG_WARPS * 32) bpe_segments_kernel(const 
         if (open >= 0 && lane == 0) emit(open, n - open);                 // (n is a multiple of 32 and the read ends open)
     };
 
-    sweep([&](int, int len) { if (len >= 2 && len <= A.giant_cap) atomicAdd(&hist[bpe_bin((uint32_t)len)], 1u); });
-    __syncthreads();
     if (!FILL) {
-        for (int i = tid; i < BPE_NB; i += blockDim.x) if (hist[i]) atomicAdd(&A.ctl[CTL_CNT + i], hist[i]);
+        sweep([&](int, int len) { if (len >= 2 && len <= A.giant_cap) atomicAdd(&hist[bpe_bin((uint32_t)len)], 1u); });
+        __syncthreads();
+        for (int i = tid; i < BPE_NB; i += blockDim.x) {
+            const uint32_t c = hist[i];
+            A.cta_hist[(size_t)blockIdx.x * BPE_NB + i] = c;
+            if (c) atomicAdd(&A.ctl[CTL_CNT + i], c);
+        }
         return;
     }
+    // the CTA's range in every bin of the list
     for (int i = tid; i < BPE_NB; i += blockDim.x) {
-        first[i] = hist[i] ? A.ctl[CTL_BASE + bpe_ord(i)] + atomicAdd(&A.ctl[CTL_FILL + i], hist[i]) : 0u;
-        hist[i] = 0u;
+        const uint32_t c = A.cta_hist[(size_t)blockIdx.x * BPE_NB + i];
+        first[i] = c ? A.ctl[CTL_BASE + bpe_ord(i)] + atomicAdd(&A.ctl[CTL_FILL + i], c) : 0u;
     }
     __syncthreads();
-    // tokens that need no merging, holes elsewhere
-    int direct = 0;
-    for (int base = 0; base < n; base += 32) {
-        const int i = base + lane;
-        if (i < n) {
-            const uint32_t c = A.cls[k0 + i];
-            A.tmp_tok[k0 + i] = (uint16_t)(c < CLS_N ? SYM_HOLE : (c == CLS_N ? SYM_N : SYM_UNK));
-            direct += c >= CLS_N;
-        }
-    }
-    __syncwarp();
     sweep([&](int start, int len) {
         if (len == 1) { A.tmp_tok[k0 + start] = (uint16_t)A.cls[k0 + start]; ++direct; return; }
         const int bin = bpe_bin((uint32_t)len);
@@ -217,12 +221,30 @@ __device__ __forceinline__ void bpe_merge_item(const BpeArgs &A, uint32_t *slice
         if (!done) {
             const uint32_t m = key >> 16;
             const int bi = (int)(key & 0xffffu);
-            int j = bi + 1;                                   // the pair's right symbol: the next alive one (it exists)
-            while ((w[j * NG] & 0xffffu) == SYM_HOLE) ++j;
-            int jn = j + 1;                                   // the alive symbol behind it, if any
-            while (jn < L && (w[jn * NG] & 0xffffu) == SYM_HOLE) ++jn;
+            // alive neighbours: four candidate positions are loaded at a time (dead runs are a few symbols long)
+            auto next_alive = [&](int from) {                 // first alive position >= from, or L
+                for (int b0 = from; b0 < L; b0 += 4) {
+                    uint32_t s4[4];
+#pragma unroll
+                    for (int x = 0; x < 4; ++x) s4[x] = w[min(b0 + x, L - 1) * NG] & 0xffffu;
+#pragma unroll
+                    for (int x = 0; x < 4; ++x) if (b0 + x < L && s4[x] != SYM_HOLE) return b0 + x;
+                }
+                return L;
+            };
+            const int j = next_alive(bi + 1);                 // the pair's right symbol (it exists)
+            const int jn = next_alive(j + 1);                 // the alive symbol behind it, if any
             int p = bi - 1;                                   // the alive symbol in front, if any
-            while (p >= 0 && (w[p * NG] & 0xffffu) == SYM_HOLE) --p;
+            for (; p >= 0; p -= 4) {
+                uint32_t s4[4];
+#pragma unroll
+                for (int x = 0; x < 4; ++x) s4[x] = w[max(p - x, 0) * NG] & 0xffffu;
+                int f = -1;
+#pragma unroll
+                for (int x = 3; x >= 0; --x) if (p - x >= 0 && s4[x] != SYM_HOLE) f = p - x;
+                if (f >= 0) { p = f; break; }
+            }
+            if (p < 0) p = -1;
             const uint32_t ns = 4u + m;
             if (g == 0) {
                 const uint32_t r1 = jn < L ? bpe_rank(A, ns, w[jn * NG] & 0xffffu) : BPE_INF;
@@ -297,26 +319,32 @@ __global__ void __launch_bounds__(32) bpe_merge_giant_kernel(const __grid_consta
     }
 }
 
-// single-block exclusive scan of per-read token counts -> out_offsets (int64), total in the last entry
+// single-block exclusive scan of per-read token counts -> out_offsets (int64), total in the last entry; four counts per
+// thread per step
 __global__ void __launch_bounds__(1024) scan_counts_kernel(const int32_t *cnt, int64_t n, int64_t *out_off) {
     __shared__ long long wsum[32];
     __shared__ long long s_carry;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     if (tid == 0) s_carry = 0;
     __syncthreads();
-    for (int64_t base = 0; base < n; base += 1024) {
-        int64_t i = base + tid;
-        long long v = (i < n) ? cnt[i] : 0, inc = v;
+    for (int64_t base = 0; base < n; base += 4096) {
+        const int64_t i = base + 4 * (int64_t)tid;
+        int v[4];
+#pragma unroll
+        for (int x = 0; x < 4; ++x) v[x] = (i + x < n) ? cnt[i + x] : 0;
+        const long long mine = (long long)v[0] + v[1] + v[2] + v[3];
+        long long inc = mine;
 #pragma unroll
         for (int d = 1; d < 32; d <<= 1) { long long t = __shfl_up_sync(0xffffffffu, inc, d); if (lane >= d) inc += t; }
         if (lane == 31) wsum[warp] = inc;
         __syncthreads();
         long long woff = 0, tot = 0;
         for (int w = 0; w < 32; ++w) { long long t = wsum[w]; if (w < warp) woff += t; tot += t; }
-        long long carry = s_carry;
-        if (i < n) out_off[i] = carry + woff + inc - v;
+        long long run = s_carry + woff + inc - mine;
+#pragma unroll
+        for (int x = 0; x < 4; ++x) { if (i + x < n) out_off[i + x] = run; run += v[x]; }
         __syncthreads();
-        if (tid == 0) s_carry = carry + tot;
+        if (tid == 0) s_carry += tot;
         __syncthreads();
     }
     if (tid == 0) out_off[n] = s_carry;

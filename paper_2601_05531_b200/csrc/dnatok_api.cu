@@ -43,6 +43,7 @@ struct EncCtx {
     int64_t *koff = nullptr; int32_t *tok_cnt = nullptr; int64_t rec_cap = 0;
     BpeSeg *segs = nullptr; int64_t segs_cap = 0;   // bin-sorted ACGT segments of 2 or more symbols
     uint32_t *bpe_ctl = nullptr;                    // bin counts, list slots, work items, work-item counters
+    uint32_t *bpe_hist = nullptr; int64_t bpe_hist_cap = 0;   // per-CTA bin counts of the segment finder
 };
 
 struct StreamSlot {
@@ -129,7 +130,7 @@ int ctx_init(dnatok_t *h, EncCtx &c) {
 void ctx_free(EncCtx &c) {
     cudaFree(c.descs); cudaFree(c.gdescs); cudaFree(c.ls); cudaFree(c.first_rec); cudaFree(c.rec_k); cudaFree(c.ticket); cudaFreeHost(c.h_status);
     cudaFree(c.prof);
-    cudaFree(c.cls); cudaFree(c.tmp_tok); cudaFree(c.koff); cudaFree(c.tok_cnt); cudaFree(c.segs); cudaFree(c.bpe_ctl);
+    cudaFree(c.cls); cudaFree(c.tmp_tok); cudaFree(c.koff); cudaFree(c.tok_cnt); cudaFree(c.segs); cudaFree(c.bpe_ctl); cudaFree(c.bpe_hist);
     c = EncCtx();
 }
 
@@ -303,12 +304,20 @@ int encode_on(dnatok_t *h, EncCtx &c, const uint8_t *d_bytes, int64_t n_bytes, c
             CU(cudaMallocAsync((void **)&c.segs, (size_t)scap * sizeof(BpeSeg), st));
             c.segs_cap = scap;
         }
+        const unsigned nb_seg = (unsigned)((n_rec + BPE_SEG_WARPS - 1) / BPE_SEG_WARPS);
+        if (c.bpe_hist_cap < (int64_t)nb_seg) {
+            if (c.bpe_hist) CU(cudaFreeAsync(c.bpe_hist, st));
+            c.bpe_hist = nullptr; c.bpe_hist_cap = 0;
+            const int64_t hcap = (int64_t)nb_seg + nb_seg / 4 + 16;
+            CU(cudaMallocAsync((void **)&c.bpe_hist, (size_t)hcap * BPE_NB * sizeof(uint32_t), st));
+            c.bpe_hist_cap = hcap;
+        }
         BpeArgs b;
+        b.cta_hist = c.bpe_hist;
         b.cls = c.cls; b.koff = c.koff; b.n_rec = n_rec; b.table = h->d_table; b.table_mask = h->table_mask;
         b.tmp_tok = c.tmp_tok; b.tok_cnt = c.tok_cnt; b.status = c.d_status;
         b.segs = c.segs; b.segs_cap = c.segs_cap; b.ctl = c.bpe_ctl; b.giant_cap = h->bpe_cap;
         CU(cudaMemsetAsync(c.bpe_ctl, 0, CTL_WORDS * sizeof(uint32_t), st));
-        const unsigned nb_seg = (unsigned)((n_rec + BPE_SEG_WARPS - 1) / BPE_SEG_WARPS);
         bpe_segments_kernel<false><<<nb_seg, BPE_SEG_WARPS * 32, 0, st>>>(b);
         bpe_bins_kernel<<<1, 128, 0, st>>>(b);
         bpe_segments_kernel<true><<<nb_seg, BPE_SEG_WARPS * 32, 0, st>>>(b);
