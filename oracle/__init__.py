@@ -18,6 +18,7 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "dnatok_oracle.c")
+_SRC_EXT = os.path.join(_HERE, "dnatok_oracle_ext.c")      # SURVEY.md 8(f) operations
 _LIB = os.path.join(_HERE, "liboracle.so")
 _lock = threading.Lock()
 _lib = None
@@ -34,9 +35,9 @@ _i32p = ctypes.POINTER(ctypes.c_int32)
 
 def build(force: bool = False) -> str:
     """Compile dnatok_oracle.c -> liboracle.so (gcc -O2) if missing or stale."""
-    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < max(os.path.getmtime(_SRC), os.path.getmtime(_SRC_EXT)):
         tmp = _LIB + f".tmp{os.getpid()}"
-        subprocess.check_call(["gcc", "-O2", "-fPIC", "-shared", "-std=c11", "-Wall", "-o", tmp, _SRC])
+        subprocess.check_call(["gcc", "-O2", "-fPIC", "-shared", "-std=c11", "-Wall", "-o", tmp, _SRC, _SRC_EXT])
         os.replace(tmp, _LIB)
     return _LIB
 
@@ -69,6 +70,21 @@ def _load():
             lib.oracle_pad.argtypes = [_i32p, _i64p, ctypes.c_int64, ctypes.c_int32, ctypes.c_int, ctypes.c_int32,
                                        _i32p, _u8p]
             lib.oracle_pad.restype = None
+            lib.oracle_kmer_table.argtypes = [_u8p, ctypes.c_int64, ctypes.c_int, _i32p, _i32p, ctypes.c_int32,
+                                              ctypes.c_int, _i32p]
+            lib.oracle_kmer_table.restype = ctypes.c_int64
+            lib.oracle_microbatch_rows.argtypes = [ctypes.c_int64] * 3
+            lib.oracle_microbatch_rows.restype = ctypes.c_int64
+            lib.oracle_embed.argtypes = [_i32p, ctypes.c_int64, _u8p, ctypes.c_int64, ctypes.c_int64, _u8p]
+            lib.oracle_embed.restype = None
+            lib.oracle_revcomp.argtypes = [_u8p, _i64p, ctypes.c_int64, _u8p]
+            lib.oracle_revcomp.restype = None
+            lib.oracle_decode.argtypes = [_i32p, _i64p, ctypes.c_int64, ctypes.c_int, ctypes.c_int, _i32p, ctypes.c_int32,
+                                          ctypes.c_int32, ctypes.c_int32, ctypes.c_int32, _i32p, ctypes.c_int32, _u8p,
+                                          ctypes.c_int64, _i64p]
+            lib.oracle_decode.restype = ctypes.c_int64
+            lib.oracle_widen.argtypes = [_i32p, ctypes.c_int64, _i64p]
+            lib.oracle_widen.restype = None
             _lib = lib
     return _lib
 
@@ -167,3 +183,87 @@ def pad(ids: np.ndarray, out_offsets: np.ndarray, cfg: Config) -> tuple[np.ndarr
     _load().oracle_pad(_p(ids, _i32p), _p(out_offsets, _i64p), n, cfg.seq_len, cfg.pad_side, cfg.pad_id,
                        _p(batch, _i32p), _p(mask, _u8p))
     return batch, mask
+
+
+# ------------------------------------------------------------------------------------------- SURVEY.md 8(f)
+def encode_kmer_table(data, offsets, cfg: Config, kmer_lut: np.ndarray) -> tuple[np.ndarray, np.ndarray]:
+    """f1: steps 1, 5 as encode(); step 3 through the base-5 table kmer_lut[5^k] (one record at a time)."""
+    if not isinstance(data, np.ndarray):
+        data = np.frombuffer(bytes(data), dtype=np.uint8)
+    data = np.ascontiguousarray(data, dtype=np.uint8)
+    offsets = np.ascontiguousarray(offsets, dtype=np.int64)
+    kl = np.ascontiguousarray(kmer_lut, dtype=np.int32)
+    assert kl.size == 5 ** cfg.k
+    nt = np.asarray(cfg.nt_ids, dtype=np.int32)
+    lut = np.ascontiguousarray(cfg.class_lut, dtype=np.uint8)
+    lib = _load()
+    parts, out = [], np.zeros(offsets.size, dtype=np.int64)
+    for r in range(offsets.size - 1):
+        rec = np.ascontiguousarray(data[int(offsets[r]): int(offsets[r + 1])])
+        cls = np.empty(max(rec.size, 1), dtype=np.uint8)
+        n = lib.oracle_strip(_p(rec if rec.size else cls, _u8p), rec.size, _p(lut, _u8p), int(cfg.strip_headers), _p(cls, _u8p))
+        ids = np.empty(max(n, 1), dtype=np.int32)
+        t = lib.oracle_kmer_table(_p(cls, _u8p), n, cfg.k, _p(kl, _i32p), _p(nt, _i32p), cfg.unk_id, cfg.tail_policy,
+                                  _p(ids, _i32p))
+        parts.append(ids[:t].copy())
+        out[r + 1] = out[r] + t
+    return (np.concatenate(parts) if parts else np.zeros(0, np.int32)), out
+
+
+def microbatch_rows(b_emb: int, m_tokens: int, t_len: int) -> int:
+    """f2: rows per embedding call, b = min(B_emb, max(1, floor(M / T')))."""
+    return int(_load().oracle_microbatch_rows(int(b_emb), int(m_tokens), int(t_len)))
+
+
+def embed(ids: np.ndarray, table: np.ndarray) -> np.ndarray:
+    """f2: out[..., :] = table[ids[...], :] (rows copied bit for bit; an ID outside the table gives a zero row)."""
+    ids32 = np.ascontiguousarray(ids, dtype=np.int32)
+    table = np.ascontiguousarray(table)
+    row_bytes = table.shape[1] * table.itemsize
+    out = np.empty(ids32.shape + (table.shape[1],), dtype=table.dtype)
+    if ids32.size:
+        _load().oracle_embed(_p(ids32, _i32p), ids32.size, _p(table.view(np.uint8).reshape(-1), _u8p), table.shape[0],
+                             row_bytes, _p(out.view(np.uint8).reshape(-1), _u8p))
+    return out
+
+
+def revcomp(data, offsets) -> np.ndarray:
+    """f3: every record reversed and complemented (same layout as the input)."""
+    if not isinstance(data, np.ndarray):
+        data = np.frombuffer(bytes(data), dtype=np.uint8)
+    data = np.ascontiguousarray(data, dtype=np.uint8)
+    offsets = np.ascontiguousarray(offsets, dtype=np.int64)
+    out = data.copy()
+    if data.size:
+        _load().oracle_revcomp(_p(data, _u8p), _p(offsets, _i64p), offsets.size - 1, _p(out, _u8p))
+    return out
+
+
+def decode(ids: np.ndarray, out_offsets: np.ndarray, cfg: Config) -> tuple[np.ndarray, np.ndarray]:
+    """f3: token IDs -> upper-case bases (uint8[total], byte_offsets int64[n_records + 1])."""
+    ids = np.ascontiguousarray(ids, dtype=np.int32)
+    out_offsets = np.ascontiguousarray(out_offsets, dtype=np.int64)
+    n = out_offsets.size - 1
+    nt = np.asarray(cfg.nt_ids, dtype=np.int32)
+    merges = np.ascontiguousarray(cfg.merges if cfg.merges is not None else np.zeros((0, 2)), dtype=np.int32).reshape(-1, 2)
+    boff = np.zeros(n + 1, dtype=np.int64)
+    cap = 1 << 16
+    idp = ids if ids.size else np.zeros(1, np.int32)
+    mp = merges if merges.size else np.zeros((1, 2), np.int32)
+    while True:
+        out = np.empty(cap, dtype=np.uint8)
+        tot = _load().oracle_decode(_p(idp, _i32p), _p(out_offsets, _i64p), n, cfg.mode, cfg.k, _p(nt, _i32p), cfg.base_id,
+                                    cfg.n_id, cfg.unk_id, cfg.pad_id, _p(mp, _i32p), merges.shape[0], _p(out, _u8p), cap,
+                                    _p(boff, _i64p))
+        if tot >= 0:
+            return out[:tot].copy(), boff
+        cap *= 4
+
+
+def widen(ids: np.ndarray) -> np.ndarray:
+    """f4: int32 IDs -> int64."""
+    ids = np.ascontiguousarray(ids, dtype=np.int32)
+    out = np.empty(ids.shape, dtype=np.int64)
+    if ids.size:
+        _load().oracle_widen(_p(ids.reshape(-1), _i32p), ids.size, _p(out.reshape(-1), _i64p))
+    return out
