@@ -165,6 +165,55 @@ int dnatok_check(dnatok_t *h, void *stream);
 /* Message for the last non-OK return on this handle (never NULL; valid until the next call on h).      */
 const char *dnatok_last_error(const dnatok_t *h);
 
+/* ---------------------------------------------------------------------------------------------------------
+ * operations next to the encoder.  All only enqueue on `stream`; none synchronises.
+ * --------------------------------------------------------------------------------------------------------- */
+
+/*
+ * dnatok_revcomp (section 4.5.4: reverse complement on device).  Record r of d_out gets record
+ * r of d_bytes reversed and complemented byte by byte: A<->T, C<->G, U->A, IUPAC R<->Y, K<->M, B<->V, D<->H;
+ * S, W, N and every other byte (line breaks included) map to themselves; case is kept.  Bytes outside every
+ * record are copied.  Meant for newline-free records (reverse complement, then dnatok_encode); d_out != d_bytes.
+ * Same d_rec_offsets contract as dnatok_encode.
+ */
+int dnatok_revcomp(dnatok_t *h, const uint8_t *d_bytes, int64_t n_bytes, const int64_t *d_rec_offsets,
+                   int64_t n_records, uint8_t *d_out, void *stream);
+
+/*
+ * dnatok_decode (section 4.5.2: decoding through an inverse vocabulary table).  Token ids of
+ * dnatok_encode / rows of dnatok_pad (CSR: d_ids of id_dtype, d_out_offsets [n_records+1]) -> upper-case bases:
+ *   single-nt: nt_ids[c] -> "ACGTN"[c], any other id -> 'N';  k-mer: base_id + code -> its k bases (first base most
+ *   significant), base_id + 4^k + c -> "ACGTN"[c], any other id (UNK) -> k x 'N';  BPE: n_id -> 'N', base_id + t ->
+ *   the spelling of token t, any other id -> 'N'.  pad_id tokens are skipped.
+ * d_byte_offsets [n_records+1] int64 gets the exclusive prefix sum of the decoded record lengths; d_bytes_out
+ * [bytes_capacity] the bytes (overflow: nothing written past the end, dnatok_check() returns DNATOK_ECAPACITY).
+ * decode(encode(x)) == upper(stripped x) whenever x holds no N and no non-DNA byte.  EINVAL on a BPE handle whose
+ * token spellings add up to more than 64 MiB.
+ */
+int dnatok_decode(dnatok_t *h, const void *d_ids, const int64_t *d_out_offsets, int64_t n_records,
+                  uint8_t *d_bytes_out, int64_t bytes_capacity, int64_t *d_byte_offsets, void *stream);
+
+/* Rows per embedding call, PAPER.md:136 (Alg. 2 l.17) / PAPER.md:181: b = min(B_emb, max(1, floor(M / T'))).   */
+int64_t dnatok_microbatch_rows(int64_t b_emb, int64_t m_tokens, int64_t t_len);
+
+/* Called after the gather of rows [first_row, first_row + n_rows) has been enqueued on `stream`.               */
+typedef void (*dnatok_microbatch_fn)(void *user, int64_t first_row, int64_t n_rows, void *d_out_rows, void *stream);
+
+/*
+ * dnatok_embed (PAPER.md:66-72 notation IDs [B x T'] -> [B x T' x D]; Alg. 2 l.18-24 micro-batch
+ * loop): d_out[r][t][:] = d_table[d_ids[r][t]][:], rows of row_bytes bytes (D x element size; a multiple of 4,
+ * 16-byte accesses when it and both pointers are multiples of 16); an id outside [0, vocab) gives a zero row.
+ * The n_rows x t_len id matrix (int32, e.g. dnatok_pad's batch_ids) is processed dnatok_microbatch_rows(b_emb,
+ * m_tokens, t_len) rows per launch, in order; on_microbatch (may be NULL) is called once per launch.  d_out holds
+ * all n_rows x t_len x row_bytes bytes.
+ */
+int dnatok_embed(dnatok_t *h, const int32_t *d_ids, int64_t n_rows, int64_t t_len, const void *d_table,
+                 int64_t vocab, int64_t row_bytes, void *d_out, int64_t b_emb, int64_t m_tokens,
+                 dnatok_microbatch_fn on_microbatch, void *user, void *stream);
+
+/* dnatok_widen_ids (IDs path "32-bit + on-device cast"): d_out[i] = (int64) d_ids[i], i < n.       */
+int dnatok_widen_ids(dnatok_t *h, const int32_t *d_ids, int64_t n, int64_t *d_out, void *stream);
+
 /* Number of kernels this library has launched on the handle since create (bench.py's gpu_launches).    */
 int64_t dnatok_launch_count(const dnatok_t *h);
 

@@ -26,6 +26,7 @@ __all__ = [
     "SINGLE_NT", "KMER", "BPE", "I16", "I32", "TAIL_PER_BASE", "TAIL_DROP", "TAIL_UNK", "PAD_LEFT", "PAD_RIGHT",
     "dnatok_create", "dnatok_destroy", "dnatok_encode", "dnatok_pad", "dnatok_stream_encode", "dnatok_check",
     "dnatok_last_error", "dnatok_launch_count", "dnatok_version", "dnatok_config_default", "dnatok_set_super_tile", "dnatok_set_grid_cap",
+    "dnatok_revcomp", "dnatok_decode", "dnatok_microbatch_rows", "dnatok_embed", "dnatok_widen_ids",
 ]
 
 SINGLE_NT, KMER, BPE = 0, 1, 2
@@ -63,6 +64,7 @@ class _CBatch(ctypes.Structure):
 
 
 _BATCH_FN = ctypes.CFUNCTYPE(None, ctypes.c_void_p, ctypes.POINTER(_CBatch))
+_MICROBATCH_FN = ctypes.CFUNCTYPE(None, ctypes.c_void_p, ctypes.c_int64, ctypes.c_int64, ctypes.c_void_p, ctypes.c_void_p)
 _lib = None
 SUPER_TILE = 0      # sub-tiles per super-tile applied to new DNATok handles (0 = automatic); a tuning knob, see dnatok.h
 GRID_CAP = 0        # cap on persistent CTAs per launch applied to new DNATok handles (0 = none); a test knob, see dnatok.h
@@ -109,6 +111,16 @@ def lib() -> ctypes.CDLL:
         L.dnatok_set_grid_cap.argtypes = [vp, i32]
         L.dnatok_launch_count.restype = i64
         L.dnatok_launch_count.argtypes = [vp]
+        L.dnatok_revcomp.restype = ctypes.c_int
+        L.dnatok_revcomp.argtypes = [vp, vp, i64, vp, i64, vp, vp]
+        L.dnatok_decode.restype = ctypes.c_int
+        L.dnatok_decode.argtypes = [vp, vp, vp, i64, vp, i64, vp, vp]
+        L.dnatok_microbatch_rows.restype = i64
+        L.dnatok_microbatch_rows.argtypes = [i64, i64, i64]
+        L.dnatok_embed.restype = ctypes.c_int
+        L.dnatok_embed.argtypes = [vp, vp, i64, i64, vp, i64, i64, vp, i64, i64, _MICROBATCH_FN, vp, vp]
+        L.dnatok_widen_ids.restype = ctypes.c_int
+        L.dnatok_widen_ids.argtypes = [vp, vp, i64, vp, vp]
         _lib = L
     return _lib
 
@@ -176,6 +188,29 @@ def dnatok_set_grid_cap(h: int, max_ctas: int) -> None:
 
 def dnatok_launch_count(h: int) -> int:
     return int(lib().dnatok_launch_count(h))
+
+
+def dnatok_revcomp(h: int, d_bytes: int, n_bytes: int, d_rec_offsets: int, n_records: int, d_out: int, stream: int = 0) -> None:
+    _chk(h, lib().dnatok_revcomp(h, d_bytes, n_bytes, d_rec_offsets, n_records, d_out, stream))
+
+
+def dnatok_decode(h: int, d_ids: int, d_out_offsets: int, n_records: int, d_bytes_out: int, bytes_capacity: int,
+                  d_byte_offsets: int, stream: int = 0) -> None:
+    _chk(h, lib().dnatok_decode(h, d_ids, d_out_offsets, n_records, d_bytes_out, bytes_capacity, d_byte_offsets, stream))
+
+
+def dnatok_microbatch_rows(b_emb: int, m_tokens: int, t_len: int) -> int:
+    return int(lib().dnatok_microbatch_rows(int(b_emb), int(m_tokens), int(t_len)))
+
+
+def dnatok_embed(h: int, d_ids: int, n_rows: int, t_len: int, d_table: int, vocab: int, row_bytes: int, d_out: int,
+                 b_emb: int, m_tokens: int, on_microbatch=None, user: int = 0, stream: int = 0) -> None:
+    cb = on_microbatch if on_microbatch is not None else _MICROBATCH_FN()
+    _chk(h, lib().dnatok_embed(h, d_ids, n_rows, t_len, d_table, vocab, row_bytes, d_out, b_emb, m_tokens, cb, user, stream))
+
+
+def dnatok_widen_ids(h: int, d_ids: int, n: int, d_out: int, stream: int = 0) -> None:
+    _chk(h, lib().dnatok_widen_ids(h, d_ids, n, d_out, stream))
 
 
 # ------------------------------------------------------------------ convenience layer
@@ -347,6 +382,45 @@ class DNATok:
         cb = _BATCH_FN(_cb)
         dnatok_stream_encode(self.h, ptr, n_bytes, offs.ctypes.data, offs.size - 1, int(chunk_bytes), int(n_streams),
                              int(max_rows_per_chunk), cb, 0)
+
+    # ---- SURVEY.md 8(f) ------------------------------------------------------------------------------
+    def revcomp(self, d_bytes, d_rec_offsets, out=None, stream=None):
+        """Reverse complement of every record (cuda uint8, same layout).  Enqueue only."""
+        t = self._torch
+        if out is None:
+            out = t.empty_like(d_bytes)
+        dnatok_revcomp(self.h, d_bytes.data_ptr(), d_bytes.numel(), d_rec_offsets.data_ptr(), d_rec_offsets.numel() - 1,
+                       out.data_ptr(), self._stream(stream))
+        return out
+
+    def decode(self, ids, out_offsets, bytes_capacity: int, stream=None):
+        """Token ids -> upper-case bases: (cuda uint8[bytes_capacity], byte_offsets int64[n_records + 1]).  Enqueue only."""
+        t = self._torch
+        n_rec = out_offsets.numel() - 1
+        out = t.empty(max(int(bytes_capacity), 1), dtype=t.uint8, device=ids.device)
+        boff = t.empty(n_rec + 1, dtype=t.int64, device=ids.device)
+        dnatok_decode(self.h, ids.data_ptr(), out_offsets.data_ptr(), n_rec, out.data_ptr(), int(bytes_capacity), boff.data_ptr(),
+                      self._stream(stream))
+        return out, boff
+
+    def embed(self, ids2d, table, b_emb: int = 4096, m_tokens: int = 1 << 20, on_microbatch=None, stream=None):
+        """out[r, t, :] = table[ids2d[r, t], :], dnatok_microbatch_rows(b_emb, m_tokens, T) rows per launch.
+        on_microbatch(first_row, n_rows) is called once per launch.  Enqueue only."""
+        t = self._torch
+        assert ids2d.dtype == t.int32 and ids2d.is_contiguous() and table.is_contiguous() and ids2d.dim() == 2
+        n_rows, T = ids2d.shape
+        out = t.empty((n_rows, T, table.shape[1]), dtype=table.dtype, device=ids2d.device)
+        cb = _MICROBATCH_FN((lambda _u, r0, n, _p, _s: on_microbatch(int(r0), int(n))) if on_microbatch else (lambda *_: None))
+        dnatok_embed(self.h, ids2d.data_ptr(), n_rows, T, table.data_ptr(), table.shape[0], table.shape[1] * table.element_size(),
+                     out.data_ptr(), int(b_emb), int(m_tokens), cb, 0, self._stream(stream))
+        return out
+
+    def widen(self, ids32, stream=None):
+        """int32 ids -> int64 (the paper's "32-bit + on-device cast").  Enqueue only."""
+        t = self._torch
+        out = t.empty(ids32.shape, dtype=t.int64, device=ids32.device)
+        dnatok_widen_ids(self.h, ids32.data_ptr(), ids32.numel(), out.data_ptr(), self._stream(stream))
+        return out
 
     def check(self, stream=None) -> None:
         """Synchronise the stream and raise DNATokError if the device status word reports a failure."""

@@ -16,6 +16,7 @@
 #include "common.cuh"
 #include "encode_v5.cuh"
 #include "encode_v7.cuh"
+#include "ext_kernels.cuh"
 #include "pad_kernel.cuh"
 
 using namespace dtk;
@@ -73,6 +74,9 @@ struct dnatok {
     EncParams prm;
     uint8_t *d_lut = nullptr;
     uint64_t *d_table = nullptr;
+    uint32_t *d_spell_off = nullptr;   // BPE decode: [4 + n_merges + 1] offsets of the token spellings
+    uint8_t *d_spell = nullptr;        //             the spellings, back to back (nullptr: too long to keep, decode unavailable)
+    int32_t *d_rec_len = nullptr; int64_t rec_len_cap = 0;   // decode: decoded bytes per record
     uint32_t table_mask = 0;
     int32_t bpe_cap = 0;
     EncCtx ctx;
@@ -516,6 +520,39 @@ int dnatok_create(const dnatok_config *cfg_in, int device, dnatok_t **out) {
         if (cudaMalloc(&h->d_table, table.size() * sizeof(uint64_t)) != cudaSuccess) return bail(DNATOK_ENOMEM);
         if (cudaMemcpy(h->d_table, table.data(), table.size() * sizeof(uint64_t), cudaMemcpyHostToDevice) != cudaSuccess)
             return bail(DNATOK_ECUDA);
+        // decode: spelling of every token (a base spells itself, token 4 + r = spelling(left) spelling(right)); kept on the
+        // device unless the spellings add up to more than 64 MiB (then dnatok_decode is unavailable on this handle)
+        {
+            const int64_t V = 4 + (int64_t)cfg.n_merges;
+            std::vector<uint32_t> off(V + 1, 0);
+            std::vector<int64_t> len(V, 1);
+            int64_t total = 4;
+            bool fits = true;
+            for (int32_t r = 0; r < cfg.n_merges && fits; ++r) {
+                len[4 + r] = len[cfg.merges[2 * r]] + len[cfg.merges[2 * r + 1]];
+                total += len[4 + r];
+                fits = total <= (64ll << 20);
+            }
+            if (fits) {
+                std::vector<uint8_t> pool((size_t)total);
+                int64_t pos = 0;
+                for (int64_t t = 0; t < V; ++t) {
+                    off[t] = (uint32_t)pos;
+                    if (t < 4) pool[pos] = (uint8_t)"ACGT"[t];
+                    else {
+                        const int32_t L = cfg.merges[2 * (t - 4)], R = cfg.merges[2 * (t - 4) + 1];
+                        memcpy(&pool[pos], &pool[off[L]], (size_t)len[L]);
+                        memcpy(&pool[pos + len[L]], &pool[off[R]], (size_t)len[R]);
+                    }
+                    pos += len[t];
+                }
+                off[V] = (uint32_t)pos;
+                if (cudaMalloc(&h->d_spell_off, off.size() * sizeof(uint32_t)) != cudaSuccess ||
+                    cudaMalloc(&h->d_spell, pool.size()) != cudaSuccess) return bail(DNATOK_ENOMEM);
+                if (cudaMemcpy(h->d_spell_off, off.data(), off.size() * sizeof(uint32_t), cudaMemcpyHostToDevice) != cudaSuccess ||
+                    cudaMemcpy(h->d_spell, pool.data(), pool.size(), cudaMemcpyHostToDevice) != cudaSuccess) return bail(DNATOK_ECUDA);
+            }
+        }
         // longest ACGT segment (run between N / UNK bytes) the merge kernels hold: up to 2048 symbols in the main kernel's
         // per-warp slice, up to BPE_GIANT_MAX in the giant kernel's (one warp per SM); longer ones are ECAPACITY
         int cap = (int)std::min<int64_t>(BPE_GIANT_MAX, std::max<int64_t>(BPE_SLOT_WORDS, (cfg.max_record_bytes + 63) & ~(int64_t)63));
@@ -566,7 +603,7 @@ int dnatok_destroy(dnatok_t *h) {
     cudaDeviceSynchronize();
     ring_free(h->ring);
     ctx_free(h->ctx);
-    cudaFree(h->d_lut); cudaFree(h->d_table);
+    cudaFree(h->d_lut); cudaFree(h->d_table); cudaFree(h->d_spell_off); cudaFree(h->d_spell); cudaFree(h->d_rec_len);
     delete h;
     return DNATOK_OK;
 }
@@ -718,6 +755,106 @@ int dnatok_debug_prof(dnatok_t *h, unsigned long long *out64) {
 #endif
 
 const char *dnatok_last_error(const dnatok_t *h) { return h ? h->err.c_str() : "null handle"; }
+
+// ---- reverse complement, decode, embedding gather, widening ------------------------------------
+int dnatok_revcomp(dnatok_t *h, const uint8_t *d_bytes, int64_t n_bytes, const int64_t *d_rec_offsets, int64_t n_records,
+                   uint8_t *d_out, void *stream) {
+    if (!h) return DNATOK_EINVAL;
+    if (n_bytes < 0 || n_records < 0 || !d_rec_offsets || (n_bytes > 0 && (!d_bytes || !d_out)) || d_bytes == d_out)
+        return fail(h, DNATOK_EINVAL, "dnatok_revcomp: bad argument (in-place is not supported)");
+    if (n_bytes == 0) return DNATOK_OK;
+    CU(cudaSetDevice(h->device));
+    RevcompArgs a{d_bytes, d_out, d_rec_offsets, n_records, n_bytes};
+    const int64_t n16 = (n_bytes + 15) >> 4;
+    int grid = (int)std::min<int64_t>((n16 + 255) / 256, (int64_t)h->sm_count * 8);
+    if (h->grid_cap > 0) grid = std::min(grid, h->grid_cap);
+    revcomp_kernel<<<grid, 256, 0, (cudaStream_t)stream>>>(a);
+    CU(cudaGetLastError());
+    h->launches += 1;
+    return DNATOK_OK;
+}
+
+int dnatok_decode(dnatok_t *h, const void *d_ids, const int64_t *d_out_offsets, int64_t n_records, uint8_t *d_bytes_out,
+                  int64_t bytes_capacity, int64_t *d_byte_offsets, void *stream) {
+    if (!h) return DNATOK_EINVAL;
+    if (n_records < 0 || bytes_capacity < 0 || !d_out_offsets || !d_byte_offsets || (bytes_capacity > 0 && !d_bytes_out))
+        return fail(h, DNATOK_EINVAL, "dnatok_decode: bad argument");
+    if (h->cfg.mode == DNATOK_BPE && !h->d_spell)
+        return fail(h, DNATOK_EINVAL, "dnatok_decode: the merge table's token spellings exceed 64 MiB");
+    CU(cudaSetDevice(h->device));
+    cudaStream_t st = (cudaStream_t)stream;
+    if (n_records + 1 > h->rec_len_cap) {
+        if (h->d_rec_len) CU(cudaFreeAsync(h->d_rec_len, st));
+        h->d_rec_len = nullptr; h->rec_len_cap = 0;
+        const int64_t cap = n_records + n_records / 4 + 256;
+        CU(cudaMallocAsync((void **)&h->d_rec_len, (size_t)cap * sizeof(int32_t), st));
+        h->rec_len_cap = cap;
+    }
+    const dnatok_config &cfg = h->cfg;
+    DecodeArgs a;
+    a.ids = d_ids; a.out_off = d_out_offsets; a.n_rec = n_records;
+    a.mode = cfg.mode; a.k = cfg.mode == DNATOK_KMER ? cfg.k : 1; a.base_id = cfg.base_id; a.n_id = cfg.n_id; a.pad_id = cfg.pad_id;
+    for (int i = 0; i < 5; ++i) a.nt_ids[i] = cfg.nt_ids[i];
+    a.four_k = 1ll << (2 * a.k);
+    a.n_tokens_bpe = 4 + cfg.n_merges; a.spell_off = h->d_spell_off; a.spell = h->d_spell;
+    a.rec_len = h->d_rec_len; a.byte_off = d_byte_offsets; a.out = d_bytes_out; a.out_cap = bytes_capacity;
+    a.status = h->ctx.d_status;
+    int grid = (int)std::min<int64_t>((n_records + 7) / 8 + 1, (int64_t)h->sm_count * 8);
+    if (h->grid_cap > 0) grid = std::min(grid, h->grid_cap);
+    const bool i16 = cfg.id_dtype == DNATOK_I16;
+    if (i16) decode_kernel<int16_t, false><<<grid, 256, 0, st>>>(a); else decode_kernel<int32_t, false><<<grid, 256, 0, st>>>(a);
+    scan_counts_kernel<<<1, 1024, 0, st>>>(h->d_rec_len, n_records, d_byte_offsets);
+    if (i16) decode_kernel<int16_t, true><<<grid, 256, 0, st>>>(a); else decode_kernel<int32_t, true><<<grid, 256, 0, st>>>(a);
+    CU(cudaGetLastError());
+    h->launches += 3;
+    return DNATOK_OK;
+}
+
+int64_t dnatok_microbatch_rows(int64_t b_emb, int64_t m_tokens, int64_t t_len) {
+    int64_t q = t_len > 0 ? m_tokens / t_len : m_tokens;
+    if (q < 1) q = 1;
+    return b_emb < q ? b_emb : q;
+}
+
+int dnatok_embed(dnatok_t *h, const int32_t *d_ids, int64_t n_rows, int64_t t_len, const void *d_table, int64_t vocab,
+                 int64_t row_bytes, void *d_out, int64_t b_emb, int64_t m_tokens, dnatok_microbatch_fn on_microbatch,
+                 void *user, void *stream) {
+    if (!h) return DNATOK_EINVAL;
+    if (n_rows < 0 || t_len <= 0 || vocab <= 0 || row_bytes <= 0 || (row_bytes & 3) || b_emb <= 0 || m_tokens <= 0 ||
+        row_bytes > (1 << 20) || (n_rows > 0 && (!d_ids || !d_table || !d_out)) ||
+        (reinterpret_cast<uintptr_t>(d_table) & 3) || (reinterpret_cast<uintptr_t>(d_out) & 3))
+        return fail(h, DNATOK_EINVAL, "dnatok_embed: bad argument (row_bytes must be a multiple of 4, buffers 4-byte aligned)");
+    CU(cudaSetDevice(h->device));
+    const bool v16 = (row_bytes & 15) == 0 && (reinterpret_cast<uintptr_t>(d_table) & 15) == 0 &&
+                     (reinterpret_cast<uintptr_t>(d_out) & 15) == 0;
+    const int64_t b = dnatok_microbatch_rows(b_emb, m_tokens, t_len);
+    for (int64_t r0 = 0; r0 < n_rows; r0 += b) {
+        const int64_t rows = std::min(b, n_rows - r0), toks = rows * t_len;
+        const int64_t acc = toks * (row_bytes / (v16 ? 16 : 4));
+        int grid = (int)std::min<int64_t>((acc + 255) / 256, (int64_t)h->sm_count * 16);
+        if (h->grid_cap > 0) grid = std::min(grid, h->grid_cap);
+        uint8_t *out = reinterpret_cast<uint8_t *>(d_out) + r0 * t_len * row_bytes;
+        if (v16) embed_kernel<16><<<grid, 256, 0, (cudaStream_t)stream>>>(d_ids + r0 * t_len, toks, (const uint8_t *)d_table, vocab, (int32_t)row_bytes, out);
+        else embed_kernel<4><<<grid, 256, 0, (cudaStream_t)stream>>>(d_ids + r0 * t_len, toks, (const uint8_t *)d_table, vocab, (int32_t)row_bytes, out);
+        CU(cudaGetLastError());
+        h->launches += 1;
+        if (on_microbatch) on_microbatch(user, r0, rows, out, stream);
+    }
+    return DNATOK_OK;
+}
+
+int dnatok_widen_ids(dnatok_t *h, const int32_t *d_ids, int64_t n, int64_t *d_out, void *stream) {
+    if (!h) return DNATOK_EINVAL;
+    if (n < 0 || (n > 0 && (!d_ids || !d_out))) return fail(h, DNATOK_EINVAL, "dnatok_widen_ids: bad argument");
+    if (n == 0) return DNATOK_OK;
+    CU(cudaSetDevice(h->device));
+    int grid = (int)std::min<int64_t>((n / 4 + 255) / 256 + 1, (int64_t)h->sm_count * 8);
+    if (h->grid_cap > 0) grid = std::min(grid, h->grid_cap);
+    widen_kernel<<<grid, 256, 0, (cudaStream_t)stream>>>(d_ids, n, d_out);
+    CU(cudaGetLastError());
+    h->launches += 1;
+    return DNATOK_OK;
+}
 
 int64_t dnatok_launch_count(const dnatok_t *h) { return h ? h->launches : 0; }
 
