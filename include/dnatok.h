@@ -83,8 +83,14 @@ typedef struct {
     int32_t  n_merges;        /*      rule r produces token 4 + r; parts must be < 4 + r, pairs unique (Q12) */
     int32_t  seq_len;         /* pad: row length of batch_ids / mask; 0 => dnatok_pad unavailable           */
     int32_t  pad_side;        /* DNATOK_PAD_LEFT (paper) | DNATOK_PAD_RIGHT                   */
-    int64_t  max_record_bytes;/* streaming / BPE: longest record in bytes the handle must be able to hold   */
-                              /* (carry buffer, per-read BPE workspace); 0 => 1 MiB                         */
+    int64_t  max_record_bytes;/* streaming: longest record in bytes the carry buffer must hold; BPE: longest */
+                              /* ACGT run between two N / UNK bytes the merge workspace must hold (runs of   */
+                              /* up to 2048 symbols always fit, at most 49152); 0 => 1 MiB                   */
+    const int32_t *kmer_lut;  /* KMER, optional (NULL: ids are the base-4 closed form): HOST pointer to the    */
+    int64_t  kmer_lut_len;    /* paper's kmer_lut[0..5^k-1] (Alg. 1 l.18-22), copied at create;   */
+                              /* must be 5^k, k <= 8.  A window's id is kmer_lut[sum_i digit_i * 5^(k-1-i)],  */
+                              /* digit = 0..3 for A,C,G,T and 4 for N and any other kept byte, so the table   */
+                              /* decides what a window holding N becomes; PER_BASE tail bases get nt_ids[c].  */
 } dnatok_config;
 
 /* Fill *cfg with the BASELINE.json vocabulary (PAD 0, UNK 1, A..T 2..5, N 6; k-mer/BPE base_id 3, n_id 2),
@@ -95,7 +101,8 @@ void dnatok_config_default(dnatok_config *cfg, int32_t mode, int32_t k);
  * dnatok_create: validate cfg, select `device`, upload LUT / merge table, allocate scan scratch.
  * EINVAL: k outside 1..15 (KMER); max id not fitting id_dtype; BPE rule referring to a token >= its own
  * product or a duplicate pair; seq_len < 0; strip_headers with class_lut['\n'] != SKIP; class_lut entry
- * not in {0..5, 255}.  On success *out owns the handle.
+ * not in {0..5, 255}; kmer_lut given with mode != KMER, k > 8, kmer_lut_len != 5^k or an id not fitting id_dtype.
+ * On success *out owns the handle.
  */
 int dnatok_create(const dnatok_config *cfg, int device, dnatok_t **out);
 int dnatok_destroy(dnatok_t *h);

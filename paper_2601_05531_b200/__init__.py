@@ -52,6 +52,7 @@ class _CConfig(ctypes.Structure):
         ("base_id", ctypes.c_int32), ("n_id", ctypes.c_int32), ("tail_policy", ctypes.c_int32),
         ("merges", ctypes.POINTER(ctypes.c_int32)), ("n_merges", ctypes.c_int32),
         ("seq_len", ctypes.c_int32), ("pad_side", ctypes.c_int32), ("max_record_bytes", ctypes.c_int64),
+        ("kmer_lut", ctypes.POINTER(ctypes.c_int32)), ("kmer_lut_len", ctypes.c_int64),
     ]
 
 
@@ -231,6 +232,7 @@ class Config:
     seq_len: int = 0
     pad_side: int = PAD_LEFT
     max_record_bytes: int = 1 << 20
+    kmer_lut: Optional[np.ndarray] = None          # KMER: int32[5^k] id table (None: base-4 closed form)
 
     def to_c(self) -> tuple[_CConfig, object]:
         mode = _MODES[self.mode] if isinstance(self.mode, str) else int(self.mode)
@@ -252,6 +254,11 @@ class Config:
             c.n_merges = int(keep.shape[0])
         c.seq_len, c.pad_side = int(self.seq_len), int(self.pad_side)
         c.max_record_bytes = int(self.max_record_bytes)
+        if self.kmer_lut is not None:
+            kl = np.ascontiguousarray(self.kmer_lut, dtype=np.int32).reshape(-1)
+            c.kmer_lut = kl.ctypes.data_as(ctypes.POINTER(ctypes.c_int32))
+            c.kmer_lut_len = int(kl.size)
+            keep = (keep, kl)
         return c, keep
 
 

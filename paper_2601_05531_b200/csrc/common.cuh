@@ -62,6 +62,9 @@ struct EncParams {
     int32_t fast_lut;       // class_lut maps ACGTacgt to 0..3 like the default: arithmetic classification is exact for them
     int32_t fast_n;         // class_lut maps 'N' and 'n' to CLS_N: runs of N can be classified arithmetically too
     uint32_t kmagic;        // floor(2^32 / k) + 1 (k >= 2): n / k == umulhi(n, kmagic) for n < 2^28
+    // table-driven k-mer ids (Alg. 1 l.18-22, kmer_lut[0..5^k-1]); both null: the base-4 closed form
+    const int32_t *kmer_lut;    // [5^k] id of every base-5 window code (digit 4 = N or any other kept byte)
+    const int32_t *remap4;      // [4^k] kmer_lut[code5(code4)]: the id of every window of A, C, G, T
 };
 
 struct EncArgs {
@@ -110,6 +113,15 @@ __device__ __forceinline__ void st_vol128(uint4 *p, uint4 v) {
 }
 
 __device__ __forceinline__ int64_t rec_pos(const EncArgs &A, int64_t r) { return A.rec_off[r] - A.off_bias + A.mis; }
+
+// table-driven id of one window: `code` = its k base-4 digits (first base most significant), `flags` = k bits, set
+// where the base is not A, C, G, T (its digit then counts as 4)
+__device__ __forceinline__ int32_t kmer_table_id(const EncParams &P, uint32_t code, uint32_t flags, int k) {
+    if (!flags) return __ldg(P.remap4 + code);
+    uint32_t c5 = 0;
+    for (int i = k - 1; i >= 0; --i) c5 = c5 * 5u + (((flags >> i) & 1u) ? 4u : ((code >> (2 * i)) & 3u));
+    return __ldg(P.kmer_lut + c5);
+}
 
 // n / k for 0 <= n < 2^28 without a divide (k = 1 passes through)
 __device__ __forceinline__ uint32_t div_k(uint32_t n, const EncParams &P) {

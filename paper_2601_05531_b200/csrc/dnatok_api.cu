@@ -74,6 +74,7 @@ struct dnatok {
     EncParams prm;
     uint8_t *d_lut = nullptr;
     uint64_t *d_table = nullptr;
+    int32_t *d_kmer_lut = nullptr, *d_remap4 = nullptr;   // table-driven k-mer ids (nullptr: base-4 closed form)
     uint32_t *d_spell_off = nullptr;   // BPE decode: [4 + n_merges + 1] offsets of the token spellings
     uint8_t *d_spell = nullptr;        //             the spellings, back to back (nullptr: too long to keep, decode unavailable)
     int32_t *d_rec_len = nullptr; int64_t rec_len_cap = 0;   // decode: decoded bytes per record
@@ -456,6 +457,7 @@ int dnatok_create(const dnatok_config *cfg_in, int device, dnatok_t **out) {
     if (cfg.id_dtype != DNATOK_I16 && cfg.id_dtype != DNATOK_I32) return DNATOK_EINVAL;
     if (cfg.seq_len < 0 || (cfg.pad_side != DNATOK_PAD_LEFT && cfg.pad_side != DNATOK_PAD_RIGHT)) return DNATOK_EINVAL;
     if (cfg.max_record_bytes <= 0) cfg.max_record_bytes = 1 << 20;
+    if (cfg.kmer_lut && cfg.mode != DNATOK_KMER) return DNATOK_EINVAL;
     int64_t max_id = std::max<int64_t>(cfg.unk_id, cfg.pad_id);
     if (cfg.mode == DNATOK_SINGLE_NT) {
         for (int i = 0; i < 5; ++i) max_id = std::max<int64_t>(max_id, cfg.nt_ids[i]);
@@ -465,6 +467,17 @@ int dnatok_create(const dnatok_config *cfg_in, int device, dnatok_t **out) {
         int64_t fk = 1ll << (2 * cfg.k);
         max_id = std::max<int64_t>(max_id, cfg.base_id + fk - 1 + (cfg.tail_policy == DNATOK_TAIL_PER_BASE ? 5 : 0));
         if (max_id > 0x7fffffffll) return DNATOK_EINVAL;
+        if (cfg.kmer_lut) {                                   // table-driven ids
+            int64_t p5 = 1;
+            for (int i = 0; i < cfg.k; ++i) p5 *= 5;
+            if (cfg.k > 8 || cfg.kmer_lut_len != p5) return DNATOK_EINVAL;
+            max_id = std::max<int64_t>(cfg.unk_id, cfg.pad_id);
+            for (int64_t i = 0; i < p5; ++i) {
+                if (cfg.kmer_lut[i] < 0) return DNATOK_EINVAL;
+                max_id = std::max<int64_t>(max_id, cfg.kmer_lut[i]);
+            }
+            for (int i = 0; i < 5; ++i) max_id = std::max<int64_t>(max_id, cfg.nt_ids[i]);
+        }
     } else {
         if (cfg.n_merges < 0 || cfg.n_merges > 65000 || (cfg.n_merges > 0 && !cfg.merges)) return DNATOK_EINVAL;
         max_id = std::max<int64_t>(max_id, std::max<int64_t>(cfg.n_id, cfg.base_id + 3 + cfg.n_merges));
@@ -493,7 +506,7 @@ int dnatok_create(const dnatok_config *cfg_in, int device, dnatok_t **out) {
 
     dnatok_t *h = new (std::nothrow) dnatok();
     if (!h) return DNATOK_ENOMEM;
-    h->cfg = cfg; h->cfg.merges = nullptr; h->device = device;
+    h->cfg = cfg; h->cfg.merges = nullptr; h->cfg.kmer_lut = nullptr; h->device = device;
     auto bail = [&](int code) { dnatok_destroy(h); return code; };
     if (cudaSetDevice(device) != cudaSuccess) return bail(DNATOK_ECUDA);
     cudaDeviceProp prop;
@@ -512,6 +525,24 @@ int dnatok_create(const dnatok_config *cfg_in, int device, dnatok_t **out) {
         if (cfg.class_lut[(uint8_t)"ACGT"[i]] != i || cfg.class_lut[(uint8_t)"acgt"[i]] != i) p.fast_lut = 0;
     p.fast_n = cfg.class_lut['N'] == DNATOK_CLS_N && cfg.class_lut['n'] == DNATOK_CLS_N;
     p.kmagic = p.k >= 2 ? (uint32_t)((1ull << 32) / (uint32_t)p.k) + 1u : 0u;
+    p.kmer_lut = nullptr; p.remap4 = nullptr;
+    if (cfg.kmer_lut) {
+        // the id of every window of A, C, G, T comes from a 4^k-entry table derived here: remap4[code4] = kmer_lut[code5(code4)]
+        const int k = cfg.k;
+        const int64_t n4 = 1ll << (2 * k);
+        std::vector<int32_t> remap((size_t)n4);
+        for (int64_t c4 = 0; c4 < n4; ++c4) {
+            int64_t c5 = 0;
+            for (int i = k - 1; i >= 0; --i) c5 = c5 * 5 + ((c4 >> (2 * i)) & 3);
+            remap[(size_t)c4] = cfg.kmer_lut[c5];
+        }
+        if (cudaMalloc(&h->d_kmer_lut, (size_t)cfg.kmer_lut_len * sizeof(int32_t)) != cudaSuccess ||
+            cudaMalloc(&h->d_remap4, (size_t)n4 * sizeof(int32_t)) != cudaSuccess) return bail(DNATOK_ENOMEM);
+        if (cudaMemcpy(h->d_kmer_lut, cfg.kmer_lut, (size_t)cfg.kmer_lut_len * sizeof(int32_t), cudaMemcpyHostToDevice) != cudaSuccess ||
+            cudaMemcpy(h->d_remap4, remap.data(), (size_t)n4 * sizeof(int32_t), cudaMemcpyHostToDevice) != cudaSuccess)
+            return bail(DNATOK_ECUDA);
+        p.kmer_lut = h->d_kmer_lut; p.remap4 = h->d_remap4;
+    }
 
     if (cudaMalloc(&h->d_lut, 256) != cudaSuccess) return bail(DNATOK_ENOMEM);
     if (cudaMemcpy(h->d_lut, cfg.class_lut, 256, cudaMemcpyHostToDevice) != cudaSuccess) return bail(DNATOK_ECUDA);
@@ -603,7 +634,7 @@ int dnatok_destroy(dnatok_t *h) {
     cudaDeviceSynchronize();
     ring_free(h->ring);
     ctx_free(h->ctx);
-    cudaFree(h->d_lut); cudaFree(h->d_table); cudaFree(h->d_spell_off); cudaFree(h->d_spell); cudaFree(h->d_rec_len);
+    cudaFree(h->d_lut); cudaFree(h->d_table); cudaFree(h->d_spell_off); cudaFree(h->d_spell); cudaFree(h->d_rec_len); cudaFree(h->d_kmer_lut); cudaFree(h->d_remap4);
     delete h;
     return DNATOK_OK;
 }
@@ -779,6 +810,7 @@ int dnatok_decode(dnatok_t *h, const void *d_ids, const int64_t *d_out_offsets, 
     if (!h) return DNATOK_EINVAL;
     if (n_records < 0 || bytes_capacity < 0 || !d_out_offsets || !d_byte_offsets || (bytes_capacity > 0 && !d_bytes_out))
         return fail(h, DNATOK_EINVAL, "dnatok_decode: bad argument");
+    if (h->d_remap4) return fail(h, DNATOK_EINVAL, "dnatok_decode: a handle with a k-mer id table has no inverse table");
     if (h->cfg.mode == DNATOK_BPE && !h->d_spell)
         return fail(h, DNATOK_EINVAL, "dnatok_decode: the merge table's token spellings exceed 64 MiB");
     CU(cudaSetDevice(h->device));

@@ -341,7 +341,7 @@ __device__ __forceinline__ void emit_group_fast(const EncArgs &A, const uint32_t
         c[t] = (s + W <= 32) ? ((a[i] >> (32 - s - W)) & ((W == 32) ? 0xffffffffu : ((1u << W) - 1u)))
                              : (__funnelshift_l(a[(i + 1 < NA) ? i + 1 : i], a[i], s) >> (32 - W));
         if (SINGLE) id[t] = affine ? P.nt_ids[0] + (int32_t)c[t] : P.nt_ids[c[t]];
-        else id[t] = P.base_id + (int32_t)c[t];
+        else id[t] = P.remap4 ? __ldg(P.remap4 + c[t]) : P.base_id + (int32_t)c[t];
     }
     if (anybad) {
 #pragma unroll
@@ -349,7 +349,7 @@ __device__ __forceinline__ void emit_group_fast(const EncArgs &A, const uint32_t
             const int bo = K * t, i = bo >> 5, s = bo & 31;
             const uint32_t m = (s + K <= 32) ? ((f[i] >> (32 - s - K)) & ((1u << K) - 1u))
                                              : (__funnelshift_l(f[(i + 1 < NF) ? i + 1 : i], f[i], s) >> (32 - K));
-            if (m) id[t] = (SINGLE && c[t] == 2u) ? P.nt_ids[4] : P.unk_id;
+            if (m) id[t] = SINGLE ? (c[t] == 2u ? P.nt_ids[4] : P.unk_id) : (P.remap4 ? kmer_table_id(P, c[t], m, K) : P.unk_id);
         }
     }
     if (sizeof(IdT) == 4) {
@@ -380,10 +380,11 @@ __device__ __forceinline__ void emit_token_slow(const EncArgs &A, const uint32_t
         id = c <= CLS_N ? P.nt_ids[c] : P.unk_id;
     } else if (jj < nwin) {
         const int u = src + jj * P.k;
-        id = flags_at(st, u, P.k) ? P.unk_id : (int32_t)(P.base_id + code_at(st, u, P.k));
+        const uint32_t fl = flags_at(st, u, P.k), cd = code_at(st, u, P.k);
+        id = P.remap4 ? kmer_table_id(P, cd, fl, P.k) : (fl ? P.unk_id : (int32_t)(P.base_id + cd));
     } else if (P.tail_policy == TAIL_PER_BASE) {
         const uint32_t c = class_at(st, src + nwin * P.k + (jj - nwin));
-        id = c <= CLS_N ? (int32_t)(P.base_id + P.four_k + c) : P.unk_id;
+        id = c <= CLS_N ? (P.remap4 ? P.nt_ids[c] : (int32_t)(P.base_id + P.four_k + c)) : P.unk_id;
     } else {
         id = P.unk_id;
     }

@@ -173,3 +173,69 @@ def test_widen(n, shift):
     got = tok.widen(cuda(a)[shift:])
     tok.check()
     assert np.array_equal(got.cpu().numpy(), oracle.widen(a[shift:]))
+
+
+# ------------------------------------------------------------------------------------------- table-driven k-mer ids (f1)
+def dense_lut():
+    lut = np.full(256, 5, dtype=np.uint8)
+    for i, (u, l) in enumerate(zip(b"ACGTN", b"acgtn")):
+        lut[u] = lut[l] = i
+    return lut
+
+
+@pytest.mark.parametrize("k,dt", [(1, 4), (2, 2), (3, 4), (6, 2), (6, 4), (8, 4)])
+@pytest.mark.parametrize("layout", ["fasta", "dense"])
+def test_kmer_table_ids(k, dt, layout):
+    """PAPER.md:88 Alg. 1 l.18-22: ids through kmer_lut[5^k]; windows holding N / other bytes take digit 4; both encoders"""
+    rng = np.random.default_rng(10 * k + dt)
+    lut5 = rng.integers(0, 30000, size=5 ** k).astype(np.int32)
+    nt = (30001, 30002, 30003, 30004, 30005)
+    if layout == "fasta":
+        w = dnagen.config3(total_bases=120_000, lo=10, hi=9000, seed=k)
+        data = w.data.copy()
+        pos = rng.integers(0, data.size, size=600)
+        data[pos[data[pos] != 10]] = rng.choice(np.frombuffer(b"NNNnRY-", dtype=np.uint8), size=int((data[pos] != 10).sum()))
+        kw, okw = {}, {}
+    else:
+        w = dnagen.config2(n_records=3)
+        data = w.data.copy()
+        data[rng.integers(0, data.size, size=300)] = ord("x")
+        kw = dict(class_lut=dense_lut(), strip_headers=False)
+        okw = dict(class_lut=dense_lut(), strip_headers=False)
+    ocfg = oracle.Config(mode=oracle.KMER, k=k, nt_ids=nt, **okw)
+    want_ids, want_off = oracle.encode_kmer_table(data, w.offsets, ocfg, lut5)
+    for S in (0, 1):
+        dn.SUPER_TILE = S
+        try:
+            tok = dn.DNATok(mode="kmer", k=k, id_dtype=dt, nt_ids=nt, kmer_lut=lut5, **kw)
+        finally:
+            dn.SUPER_TILE = 0
+        ids, out = tok.encode(cuda(data), cuda(w.offsets))
+        tok.check()
+        out = out.cpu().numpy()
+        assert np.array_equal(out, want_off)
+        assert np.array_equal(ids[: out[-1]].cpu().numpy().astype(np.int32), want_ids)
+
+
+def test_kmer_table_closed_form_table_reproduces_the_default_ids_and_bad_tables_are_rejected():
+    k = 4
+    lut5 = np.empty(5 ** k, dtype=np.int32)
+    for code in range(5 ** k):
+        d = [(code // 5 ** (k - 1 - i)) % 5 for i in range(k)]
+        lut5[code] = 1 if 4 in d else 3 + sum(x * 4 ** (k - 1 - i) for i, x in enumerate(d))
+    w = dnagen.config1()
+    d, o = cuda(w.data), cuda(w.offsets)
+    a = dn.DNATok(mode="kmer", k=k)
+    b = dn.DNATok(mode="kmer", k=k, kmer_lut=lut5, nt_ids=tuple(3 + 4 ** k + c for c in range(5)))
+    ia, oa = a.encode(d, o)
+    ib, ob = b.encode(d, o)
+    a.check(); b.check()
+    n = int(oa[-1])
+    assert torch.equal(oa, ob) and torch.equal(ia[:n], ib[:n])
+    for bad in (dict(mode="kmer", k=4, kmer_lut=lut5[:-1]), dict(mode="kmer", k=9, kmer_lut=np.zeros(5 ** 9, np.int32)),
+                dict(mode="single_nt", kmer_lut=lut5), dict(mode="kmer", k=4, id_dtype=dn.I16, kmer_lut=lut5 + 40000)):
+        with pytest.raises(dn.DNATokError) as e:
+            dn.DNATok(**bad)
+        assert e.value.code == dn.EINVAL
+    with pytest.raises(dn.DNATokError):
+        b.decode(ib, ob, bytes_capacity=10)
