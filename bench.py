@@ -565,6 +565,67 @@ def bench_config(dn, torch, D: Dist, local: int, config: int, k: int, args, *, e
     return res
 
 
+def ablation(dn, torch, local: int, args) -> dict:
+    """the paper's IDs path next to the bytes path, in the shape of its Table S2:
+    int64 vs int32 + on-device widening for the host-mapped IDs path, and 1 vs n_streams streams for the bytes
+    path.  Workload: equal-length clean strings as in the paper's microbenchmarks -- B rows of T = 512
+    uniform-ACGT bases, single-nucleotide vocabulary.  Every arm is timed end to end from HOST memory (host clock around
+    enqueue .. synchronize, median of 3 after one warm-up); the host LUT map of the IDs path is numpy fancy indexing on one
+    thread, as in the paper ("vectorised CPU map")."""
+    T = 512
+    B = max(1, int(args.ablation_mib * MIB) // T)
+    n = B * T
+    rng = np.random.default_rng(7)
+    pin_bytes = torch.empty(n, dtype=torch.uint8).pin_memory()
+    pin_bytes.numpy()[:] = np.frombuffer(b"ACGT", dtype=np.uint8)[rng.integers(0, 4, size=n)]
+    offsets = (np.arange(B + 1, dtype=np.int64) * T)
+    lut_ids = np.full(256, 1, dtype=np.int64)                       # ASCII -> id, the IDs path's host table (PAPER.md:88)
+    for i, (u, l) in enumerate(zip(b"ACGTN", b"acgtn")):
+        lut_ids[u] = lut_ids[l] = 2 + i
+    lut32 = lut_ids.astype(np.int32)
+    pin64 = torch.empty(n, dtype=torch.int64).pin_memory()
+    pin32 = torch.empty(n, dtype=torch.int32).pin_memory()
+    d64 = torch.empty(n, dtype=torch.int64, device="cuda")
+    d32 = torch.empty(n, dtype=torch.int32, device="cuda")
+    d_bytes = torch.empty(n, dtype=torch.uint8, device="cuda")
+    d_off = torch.from_numpy(offsets).cuda()
+    tok = dn.DNATok(mode="single_nt", class_lut=dense_lut(), strip_headers=False, max_record_bytes=65536, device=local)
+    ids = torch.empty(n + 64, dtype=torch.int32, device="cuda")
+    out_off = torch.empty(B + 1, dtype=torch.int64, device="cuda")
+    src = pin_bytes.numpy()
+
+    def ids64():
+        np.take(lut_ids, src, out=pin64.numpy()); d64.copy_(pin64, non_blocking=True)
+
+    def ids32():
+        np.take(lut32, src, out=pin32.numpy()); d32.copy_(pin32, non_blocking=True); tok.widen(d32)
+
+    def bytes_resident():
+        d_bytes.copy_(pin_bytes, non_blocking=True); tok.encode(d_bytes, d_off, ids_out=ids, out_offsets=out_off)
+
+    def bytes_stream(ns):
+        return lambda: tok.stream_encode(pin_bytes, offsets, args.chunk_mib * MIB, ns, max_rows_per_chunk=args.chunk_mib * MIB // T + 2)
+
+    def timed(fn):
+        fn(); torch.cuda.synchronize()
+        ts = []
+        for _ in range(3):
+            t0 = time.perf_counter(); fn(); torch.cuda.synchronize(); ts.append(time.perf_counter() - t0)
+        return float(np.median(ts))
+
+    arms = {"ids_path_int64": timed(ids64), "ids_path_int32_widen_on_device": timed(ids32),
+            "bytes_path_one_copy_then_encode": timed(bytes_resident),
+            "bytes_path_stream_1": timed(bytes_stream(1)), f"bytes_path_stream_{args.streams}": timed(bytes_stream(args.streams))}
+    # the three paths must agree on the ids (checked once, untimed)
+    tok.check()
+    same = bool(torch.equal(d64, tok.widen(d32))) and bool(torch.equal(d64[: n], ids[: n].to(torch.int64)))
+    base = arms["ids_path_int64"]
+    return {"workload": f"{B} rows x {T} uniform-ACGT bases, single-nt vocabulary (PAPER.md Table S2 shape)", "tokens": n,
+            "tokens_per_s": {k: n / v for k, v in arms.items()}, "speedup_vs_ids_int64": {k: base / v for k, v in arms.items()},
+            "seconds": arms, "ids_agree": same, "host_map": "numpy.take on 1 thread",
+            "note": "IDs path = host LUT map -> pinned ids -> H2D (PAPER.md:82); bytes path = raw bytes -> H2D -> device LUT (PAPER.md:84)"}
+
+
 def run_ours(args) -> None:
     import torch
     import paper_2601_05531_b200 as dn
@@ -601,6 +662,10 @@ def run_ours(args) -> None:
             if c != 3:
                 keep3.clear()                                            # free the 1 GiB sweep input before the big configs
             del r
+    abl = None
+    if rank0 and single and args.ablation and not args.only:
+        abl = ablation(dn, torch, local, args)
+        bad = bad or not abl["ids_agree"]
     D.close()
     if not rank0:
         return
@@ -615,7 +680,7 @@ def run_ours(args) -> None:
         "roofline": head["roofline"], "cpu_baseline": cpu, "e2e": e2e,
         "gpu_launches": head["gpu_launches"] + sum(c["gpu_launches"] for c in configs.values()),
         "launches_per_step": head["launches_per_step"], "clocks": head["clocks"], "parity": head["parity"],
-        "ms_per_step_stats": head["ms_per_step_stats"], "configs": configs,
+        "ms_per_step_stats": head["ms_per_step_stats"], "configs": configs, "ablation": abl,
         "context": "paper (H200, IDs path + embedding): 1.93-2.18e8 tokens/s encode, 1.27-1.84e8 e2e; not comparable",
     }
     if "strong" in head:
@@ -664,6 +729,8 @@ def main() -> None:
     ap.add_argument("--super-tile", type=int, default=0, help="tuning: 16 KiB units per tile (0 = automatic)")
     ap.add_argument("--no-dense", action="store_true", help="configs 2 and 4: default table (with SKIP) instead of the dense spec")
     ap.add_argument("--full-parity", action="store_true", help="compare every id of every config with the oracle")
+    ap.add_argument("--no-ablation", dest="ablation", action="store_false", help="skip the IDs-path / streams ablation (SURVEY 8(f) f4)")
+    ap.add_argument("--ablation-mib", type=int, default=128, help="tokens of the ablation workload, in Mi")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--no-parity", action="store_true")

@@ -123,6 +123,11 @@ __device__ __forceinline__ int32_t kmer_table_id(const EncParams &P, uint32_t co
     return __ldg(P.kmer_lut + c5);
 }
 
+// the same, out of line: for the token-at-a-time paths of the per-k kernels, whose loops are sensitive to their footprint
+__device__ __noinline__ int32_t kmer_table_id_cold(const EncParams &P, uint32_t code, uint32_t flags, int k) {
+    return kmer_table_id(P, code, flags, k);
+}
+
 // n / k for 0 <= n < 2^28 without a divide (k = 1 passes through)
 __device__ __forceinline__ uint32_t div_k(uint32_t n, const EncParams &P) {
     return P.k == 1 ? n : __umulhi(n, P.kmagic);

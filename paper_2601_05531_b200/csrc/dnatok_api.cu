@@ -239,7 +239,8 @@ int launch_tiles(dnatok_t *h, EncCtx &c, const EncParams &prm, const uint8_t *d_
     a.status = c.d_status; a.prof = c.prof; a.gen = c.gen; a.n_tiles = (int32_t)n_tiles; a.prm = prm;
     int grid = (int)std::min<int64_t>(n_tiles, slots);
     if (h->grid_cap > 0) grid = std::min(grid, h->grid_cap);
-    const int kk = prm.mode == MODE_KMER ? prm.k : 0;
+    // table-driven ids are compiled into the run-time-switch variant only (the per-k variants stay lean)
+    const int kk = prm.mode == MODE_KMER ? (prm.remap4 ? 99 : prm.k) : 0;
     const unsigned nb_first = (unsigned)((n_tiles + 1 + 255) / 256);
     if (dense) {
         // record range of every tile + out_offsets (closed form from the record lengths), one launch

@@ -269,7 +269,7 @@ struct SegTab { const int32_t *src, *t, *nwin; };
 // One group = R = 16 / sizeof(IdT) consecutive output slots, aligned to 16 bytes in ids_out.  A thread that
 // owns a full group inside the window part of one segment reads the stream words once, aligns them with one
 // funnel shift per word and cuts R windows at compile-time offsets; everything else goes one token at a time.
-template <typename IdT, int K, bool SINGLE>
+template <typename IdT, int K, bool SINGLE, bool REMAP = false>
 __device__ __forceinline__ void emit_group_fast(const EncArgs &A, const uint32_t *st, int u, IdT *dst, bool affine) {
     constexpr int R = 16 / (int)sizeof(IdT);
     constexpr int W = 2 * K;                             // code bits per token
@@ -308,7 +308,7 @@ __device__ __forceinline__ void emit_group_fast(const EncArgs &A, const uint32_t
         c[t] = (s + W <= 32) ? ((a[i] >> (32 - s - W)) & ((W == 32) ? 0xffffffffu : ((1u << W) - 1u)))
                              : (__funnelshift_l(a[(i + 1 < NA) ? i + 1 : i], a[i], s) >> (32 - W));
         if (SINGLE) id[t] = affine ? P.nt_ids[0] + (int32_t)c[t] : P.nt_ids[c[t]];
-        else id[t] = P.remap4 ? __ldg(P.remap4 + c[t]) : P.base_id + (int32_t)c[t];
+        else id[t] = (REMAP && P.remap4) ? __ldg(P.remap4 + c[t]) : P.base_id + (int32_t)c[t];
     }
     if (anybad) {
 #pragma unroll
@@ -316,7 +316,7 @@ __device__ __forceinline__ void emit_group_fast(const EncArgs &A, const uint32_t
             const int bo = K * t, i = bo >> 5, s = bo & 31;
             const uint32_t m = (s + K <= 32) ? ((f[i] >> (32 - s - K)) & ((1u << K) - 1u))
                                              : (__funnelshift_l(f[(i + 1 < NF) ? i + 1 : i], f[i], s) >> (32 - K));
-            if (m) id[t] = SINGLE ? (c[t] == 2u ? P.nt_ids[4] : P.unk_id) : (P.remap4 ? kmer_table_id(P, c[t], m, K) : P.unk_id);
+            if (m) id[t] = SINGLE ? (c[t] == 2u ? P.nt_ids[4] : P.unk_id) : ((REMAP && P.remap4) ? kmer_table_id(P, c[t], m, K) : P.unk_id);
         }
     }
     if (sizeof(IdT) == 4) {
@@ -348,7 +348,7 @@ __device__ __forceinline__ void emit_token_slow(const EncArgs &A, const uint32_t
     } else if (jj < nwin) {
         const int u = src + jj * P.k;
         const uint32_t fl = flags_at(st, u, P.k), cd = code_at(st, u, P.k);
-        id = P.remap4 ? kmer_table_id(P, cd, fl, P.k) : (fl ? P.unk_id : (int32_t)(P.base_id + cd));
+        id = P.remap4 ? kmer_table_id_cold(P, cd, fl, P.k) : (fl ? P.unk_id : (int32_t)(P.base_id + cd));
     } else if (P.tail_policy == TAIL_PER_BASE) {
         const uint32_t c = class_at(st, src + nwin * P.k + (jj - nwin));
         id = c <= CLS_N ? (P.remap4 ? P.nt_ids[c] : (int32_t)(P.base_id + P.four_k + c)) : P.unk_id;
@@ -394,13 +394,13 @@ __device__ __forceinline__ void emit_range(const EncArgs &A, const uint32_t *st,
             else if constexpr (KK > 0) emit_group_fast<IdT, KK, false>(A, st, u, dst, false);
             else switch (kk) {
                 case 0: emit_group_fast<IdT, 1, true>(A, st, u, dst, affine); break;
-                case 1: emit_group_fast<IdT, 1, false>(A, st, u, dst, false); break;
-                case 2: emit_group_fast<IdT, 2, false>(A, st, u, dst, false); break;
-                case 3: emit_group_fast<IdT, 3, false>(A, st, u, dst, false); break;
-                case 4: emit_group_fast<IdT, 4, false>(A, st, u, dst, false); break;
-                case 5: emit_group_fast<IdT, 5, false>(A, st, u, dst, false); break;
-                case 6: emit_group_fast<IdT, 6, false>(A, st, u, dst, false); break;
-                default: emit_group_fast<IdT, 8, false>(A, st, u, dst, false); break;
+                case 1: emit_group_fast<IdT, 1, false, true>(A, st, u, dst, false); break;
+                case 2: emit_group_fast<IdT, 2, false, true>(A, st, u, dst, false); break;
+                case 3: emit_group_fast<IdT, 3, false, true>(A, st, u, dst, false); break;
+                case 4: emit_group_fast<IdT, 4, false, true>(A, st, u, dst, false); break;
+                case 5: emit_group_fast<IdT, 5, false, true>(A, st, u, dst, false); break;
+                case 6: emit_group_fast<IdT, 6, false, true>(A, st, u, dst, false); break;
+                default: emit_group_fast<IdT, 8, false, true>(A, st, u, dst, false); break;
             }
         } else {
             for (int j = lo; j < hi; ++j) {
@@ -412,13 +412,13 @@ __device__ __forceinline__ void emit_range(const EncArgs &A, const uint32_t *st,
 }
 
 // fast groups [qa, qb) of one segment: group q holds tokens q * R - a + (0 .. R-1); token t_lo starts at stream position u0
-template <typename IdT, int K, bool SINGLE>
+template <typename IdT, int K, bool SINGLE, bool REMAP = false>
 __device__ __forceinline__ void emit_fast_groups(const EncArgs &A, const uint32_t *st, int qa, int qb, int u0, int a, int t_lo,
                                                  IdT *idsA, bool affine) {
     constexpr int R = 16 / (int)sizeof(IdT);
     constexpr int KS = SINGLE ? 1 : K;
     for (int q = qa + (int)threadIdx.x; q < qb; q += NT)
-        emit_group_fast<IdT, K, SINGLE>(A, st, u0 + (q * R - a - t_lo) * KS, idsA + q * R, affine);
+        emit_group_fast<IdT, K, SINGLE, REMAP>(A, st, u0 + (q * R - a - t_lo) * KS, idsA + q * R, affine);
 }
 
 // all tokens [0, ntok) of a short segment table (at most EVW + 1 entries): per segment, the 16-byte groups that lie
@@ -445,13 +445,13 @@ __device__ __forceinline__ void emit_segments(const EncArgs &A, const uint32_t *
             else if constexpr (KK > 0) emit_fast_groups<IdT, KK, false>(A, st, qa, qb, u0, a, t_lo, idsA, false);
             else switch (kk) {
                 case 0: emit_fast_groups<IdT, 1, true>(A, st, qa, qb, u0, a, t_lo, idsA, affine); break;
-                case 1: emit_fast_groups<IdT, 1, false>(A, st, qa, qb, u0, a, t_lo, idsA, false); break;
-                case 2: emit_fast_groups<IdT, 2, false>(A, st, qa, qb, u0, a, t_lo, idsA, false); break;
-                case 3: emit_fast_groups<IdT, 3, false>(A, st, qa, qb, u0, a, t_lo, idsA, false); break;
-                case 4: emit_fast_groups<IdT, 4, false>(A, st, qa, qb, u0, a, t_lo, idsA, false); break;
-                case 5: emit_fast_groups<IdT, 5, false>(A, st, qa, qb, u0, a, t_lo, idsA, false); break;
-                case 6: emit_fast_groups<IdT, 6, false>(A, st, qa, qb, u0, a, t_lo, idsA, false); break;
-                default: emit_fast_groups<IdT, 8, false>(A, st, qa, qb, u0, a, t_lo, idsA, false); break;
+                case 1: emit_fast_groups<IdT, 1, false, true>(A, st, qa, qb, u0, a, t_lo, idsA, false); break;
+                case 2: emit_fast_groups<IdT, 2, false, true>(A, st, qa, qb, u0, a, t_lo, idsA, false); break;
+                case 3: emit_fast_groups<IdT, 3, false, true>(A, st, qa, qb, u0, a, t_lo, idsA, false); break;
+                case 4: emit_fast_groups<IdT, 4, false, true>(A, st, qa, qb, u0, a, t_lo, idsA, false); break;
+                case 5: emit_fast_groups<IdT, 5, false, true>(A, st, qa, qb, u0, a, t_lo, idsA, false); break;
+                case 6: emit_fast_groups<IdT, 6, false, true>(A, st, qa, qb, u0, a, t_lo, idsA, false); break;
+                default: emit_fast_groups<IdT, 8, false, true>(A, st, qa, qb, u0, a, t_lo, idsA, false); break;
             }
             const int h1 = min(t_hi, qa * R - a), h2 = max(t_lo, qb * R - a);     // tokens before / after the fast groups
             const int n1 = h1 - t_lo, n2 = t_hi - h2;

@@ -368,7 +368,7 @@ __device__ __noinline__ void emit_generic(const EncArgs &A, const uint32_t *st, 
             if (P.remap4) {
                 uint32_t fl = 0;
                 for (int i = 0; i < k; ++i) fl = (fl << 1) | flags_at(st, slot_of(tb, src + jj * k + i), 1);
-                id = kmer_table_id(P, code, fl, k);
+                id = kmer_table_id_cold(P, code, fl, k);
             } else id = bad ? P.unk_id : (int32_t)(P.base_id + code);
         } else if (P.tail_policy == TAIL_PER_BASE) {
             const uint32_t c = class_at(st, slot_of(tb, src + nwin * k + (jj - nwin)));
