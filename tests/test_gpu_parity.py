@@ -1,5 +1,6 @@
 """GPU parity: the CUDA path (through the C-ABI) against the CPU oracle, bit-exact, ID for ID and offset
-for offset, on seeded inputs.  Small shapes span several 8 KiB tiles and ragged tails; edge cases cover
+for offset, on seeded inputs.  Small shapes span several 16 KiB sub-tiles and ragged tails (tests/test_gpu_fullsize.py
+holds the full-size configs); edge cases cover
 empty / tiny / huge records, headers across tiles, unaligned pointers and capacity overflow."""
 import json
 import os
