@@ -147,23 +147,39 @@ typedef struct {
 typedef void (*dnatok_batch_fn)(void *user, const dnatok_batch *batch);
 
 /*
- * dnatok_stream_encode: step 7.  Splits the PINNED host buffer into chunk_bytes pieces; chunk i goes to
+ * dnatok_stream_encode: step 7.  Splits the host buffer into chunk_bytes pieces; chunk i goes to
  * device slot i mod n_streams on its own stream: H2D copy, carry of the record cut by the previous chunk
  * boundary, steps 1-6.  H2D of chunk i+1 overlaps the encode of chunk i.  Output equals dnatok_encode
  * (+ dnatok_pad) on the whole buffer, delivered batch by batch in record order; a record is delivered in
  * the chunk where it ends.  on_batch is called on the calling thread right after the batch's work has been
  * enqueued on batch->stream (enqueue consumer work there; the slot is recycled n_streams chunks later,
  * after that stream's work).  Returns after the last chunk has completed.
- *   h_pinned       [n_bytes] page-locked host memory (cudaHostAlloc / cudaHostRegister / torch pin_memory)
+ *   h_bytes        [n_bytes] host memory.  Page-locked (cudaHostAlloc / cudaHostRegister / torch pin_memory): the
+ *                  copies read it in place.  Pageable: every chunk is first copied into one of n_streams + 1 pinned
+ *                  staging slots the handle owns (PAPER.md:181 persistent pinned buffers), at memcpy speed.
  *   h_rec_offsets  [n_records+1] host int64, same contract as dnatok_encode
  *   max_rows_per_chunk  upper bound on records ending in one chunk (sizes the per-slot batch tensors);
  *                  0 => chunk_bytes / 64 + 2.  Exceeding it returns DNATOK_ECAPACITY.
  * A record longer than cfg.max_record_bytes + chunk_bytes returns DNATOK_ECAPACITY.
  */
-int dnatok_stream_encode(dnatok_t *h, const uint8_t *h_pinned, int64_t n_bytes,
+int dnatok_stream_encode(dnatok_t *h, const uint8_t *h_bytes, int64_t n_bytes,
                          const int64_t *h_rec_offsets, int64_t n_records,
                          int64_t chunk_bytes, int n_streams, int64_t max_rows_per_chunk,
                          dnatok_batch_fn on_batch, void *user);
+
+/*
+ * dnatok_stream_encode_from: the same with a PRODUCER instead of a buffer (a file reader, a decompressor).  For chunk i
+ * the library calls fill(fill_user, i, offset, n, dst) on the calling thread; it must write bytes [offset, offset + n)
+ * of the input to dst, a pinned staging slot (n_streams + 1 of them, so the producer of chunk i + 1 runs while the
+ * copies and kernels of chunks i, i - 1, ... are in flight), and return 0; any other value aborts with EINVAL.
+ * h_rec_offsets as above (known up front, e.g. from a .fai index).
+ * On any failure of either call the ring's streams are drained before the call returns.
+ */
+typedef int (*dnatok_fill_fn)(void *fill_user, int64_t chunk_index, int64_t offset, int64_t n_bytes, uint8_t *dst);
+int dnatok_stream_encode_from(dnatok_t *h, dnatok_fill_fn fill, void *fill_user, int64_t n_bytes,
+                              const int64_t *h_rec_offsets, int64_t n_records,
+                              int64_t chunk_bytes, int n_streams, int64_t max_rows_per_chunk,
+                              dnatok_batch_fn on_batch, void *user);
 
 /* Synchronise `stream` and report the handle's device status word: DNATOK_OK, DNATOK_ECAPACITY or
  * DNATOK_ESTATE (sticky until read).                                                                  */

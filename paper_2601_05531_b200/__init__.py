@@ -26,7 +26,7 @@ __all__ = [
     "SINGLE_NT", "KMER", "BPE", "I16", "I32", "TAIL_PER_BASE", "TAIL_DROP", "TAIL_UNK", "PAD_LEFT", "PAD_RIGHT",
     "dnatok_create", "dnatok_destroy", "dnatok_encode", "dnatok_pad", "dnatok_stream_encode", "dnatok_check",
     "dnatok_last_error", "dnatok_launch_count", "dnatok_version", "dnatok_config_default", "dnatok_set_super_tile", "dnatok_set_grid_cap",
-    "dnatok_revcomp", "dnatok_decode", "dnatok_microbatch_rows", "dnatok_embed", "dnatok_widen_ids",
+    "dnatok_stream_encode_from", "dnatok_revcomp", "dnatok_decode", "dnatok_microbatch_rows", "dnatok_embed", "dnatok_widen_ids",
 ]
 
 SINGLE_NT, KMER, BPE = 0, 1, 2
@@ -65,6 +65,7 @@ class _CBatch(ctypes.Structure):
 
 
 _BATCH_FN = ctypes.CFUNCTYPE(None, ctypes.c_void_p, ctypes.POINTER(_CBatch))
+_FILL_FN = ctypes.CFUNCTYPE(ctypes.c_int, ctypes.c_void_p, ctypes.c_int64, ctypes.c_int64, ctypes.c_int64, ctypes.c_void_p)
 _MICROBATCH_FN = ctypes.CFUNCTYPE(None, ctypes.c_void_p, ctypes.c_int64, ctypes.c_int64, ctypes.c_void_p, ctypes.c_void_p)
 _lib = None
 SUPER_TILE = 0      # sub-tiles per super-tile applied to new DNATok handles (0 = automatic); a tuning knob, see dnatok.h
@@ -102,6 +103,8 @@ def lib() -> ctypes.CDLL:
         L.dnatok_pad.argtypes = [vp, vp, vp, i64, vp, vp, vp]
         L.dnatok_stream_encode.restype = ctypes.c_int
         L.dnatok_stream_encode.argtypes = [vp, vp, i64, vp, i64, i64, ctypes.c_int, i64, _BATCH_FN, vp]
+        L.dnatok_stream_encode_from.restype = ctypes.c_int
+        L.dnatok_stream_encode_from.argtypes = [vp, _FILL_FN, vp, i64, vp, i64, i64, ctypes.c_int, i64, _BATCH_FN, vp]
         L.dnatok_check.restype = ctypes.c_int
         L.dnatok_check.argtypes = [vp, vp]
         L.dnatok_last_error.restype = ctypes.c_char_p
@@ -169,6 +172,12 @@ def dnatok_stream_encode(h: int, h_pinned: int, n_bytes: int, h_rec_offsets: int
                          chunk_bytes: int, n_streams: int, max_rows_per_chunk: int, on_batch, user: int = 0) -> None:
     _chk(h, lib().dnatok_stream_encode(h, h_pinned, n_bytes, h_rec_offsets, n_records, chunk_bytes, n_streams,
                                        max_rows_per_chunk, on_batch, user))
+
+
+def dnatok_stream_encode_from(h: int, fill, fill_user: int, n_bytes: int, h_rec_offsets: int, n_records: int,
+                              chunk_bytes: int, n_streams: int, max_rows_per_chunk: int, on_batch, user: int = 0) -> None:
+    _chk(h, lib().dnatok_stream_encode_from(h, fill, fill_user, n_bytes, h_rec_offsets, n_records, chunk_bytes, n_streams,
+                                            max_rows_per_chunk, on_batch, user))
 
 
 def dnatok_check(h: int, stream: int = 0) -> None:
@@ -366,10 +375,36 @@ class DNATok:
         ids, off = self.encode(d_bytes, d_rec_offsets, stream=stream)
         return self.pad(ids, off, stream=stream)
 
+    def _batch_cb(self, on_batch):
+        cfg = self.cfg
+
+        def _cb(_user, bp):
+            b = bp.contents
+            if on_batch is not None:
+                on_batch(Batch(b.first_record, b.n_records, b.chunk_index, b.stream or 0, b.d_ids or 0,
+                               b.d_out_offsets or 0, b.d_batch_ids or 0, b.d_mask or 0, cfg.seq_len, cfg.id_dtype))
+        return _BATCH_FN(_cb)
+
+    def stream_encode_from(self, fill: Callable[[int, int, np.ndarray], None], n_bytes: int, h_rec_offsets, chunk_bytes: int,
+                           n_streams: int = 4, max_rows_per_chunk: int = 0, on_batch: Callable[[Batch], None] | None = None) -> None:
+        """Step 7 with a producer: fill(chunk_index, offset, dst) writes input bytes [offset, offset + dst.size) into dst, a
+        numpy view of one of the handle's pinned staging slots (e.g. f.readinto(dst))."""
+        offs = np.ascontiguousarray(np.asarray(h_rec_offsets), dtype=np.int64)
+
+        def _fill(_user, i, off, n, dst):
+            try:
+                fill(int(i), int(off), np.ctypeslib.as_array(ctypes.cast(dst, ctypes.POINTER(ctypes.c_uint8)), shape=(int(n),)))
+                return 0
+            except Exception:
+                return 1
+
+        dnatok_stream_encode_from(self.h, _FILL_FN(_fill), 0, int(n_bytes), offs.ctypes.data, offs.size - 1, int(chunk_bytes),
+                                  int(n_streams), int(max_rows_per_chunk), self._batch_cb(on_batch), 0)
+
     def stream_encode(self, h_pinned, h_rec_offsets, chunk_bytes: int, n_streams: int = 4,
                       max_rows_per_chunk: int = 0, on_batch: Callable[[Batch], None] | None = None) -> None:
-        """Step 7.  h_pinned: pinned CPU uint8 tensor (or numpy array over pinned memory); h_rec_offsets: CPU
-        int64 tensor / numpy array.  on_batch(Batch) runs on this thread per chunk."""
+        """Step 7.  h_pinned: CPU uint8 tensor or numpy array, pinned (read in place) or pageable (staged through the handle's
+        pinned ring); h_rec_offsets: CPU int64 tensor / numpy array.  on_batch(Batch) runs on this thread per chunk."""
         t = self._torch
         if isinstance(h_pinned, t.Tensor):
             assert h_pinned.dtype == t.uint8 and not h_pinned.is_cuda and h_pinned.is_contiguous()

@@ -7,6 +7,7 @@
 
 #include <algorithm>
 #include <cstdarg>
+#include <cstdint>
 #include <cstdio>
 #include <cstring>
 #include <string>
@@ -63,6 +64,9 @@ struct StreamRing {
     int n_streams = 0, n_slots = 0;
     std::vector<cudaStream_t> streams;
     std::vector<StreamSlot> slots;
+    // pinned staging ring for a producer that reads from a file or from pageable memory: n_streams + 1 slots of chunk_bytes
+    std::vector<uint8_t *> stage;
+    std::vector<cudaEvent_t> ev_stage;           // the H2D copy out of the slot has finished
 };
 
 }  // namespace
@@ -100,6 +104,17 @@ int fail(dnatok_t *h, int code, const char *fmt, ...) {
     }
     return code;
 }
+
+// selects the handle's device for the duration of an entry point and gives the caller's device back afterwards
+struct DeviceGuard {
+    int prev = -1, cur = -1;
+    bool ok = false;
+    explicit DeviceGuard(int d) : cur(d) { ok = cudaGetDevice(&prev) == cudaSuccess && (prev == d || cudaSetDevice(d) == cudaSuccess); }
+    ~DeviceGuard() { if (prev >= 0 && prev != cur) cudaSetDevice(prev); }
+    DeviceGuard(const DeviceGuard &) = delete;
+    DeviceGuard &operator=(const DeviceGuard &) = delete;
+};
+#define USE_DEVICE(h) DeviceGuard dev_guard_((h)->device); if (!dev_guard_.ok) return fail((h), DNATOK_ECUDA, "cannot select device %d", (h)->device)
 
 #define CU(call)                                                                                      \
     do {                                                                                              \
@@ -358,11 +373,12 @@ int encode_on(dnatok_t *h, EncCtx &c, const uint8_t *d_bytes, int64_t n_bytes, c
 }
 
 int pad_on(dnatok_t *h, const void *d_ids, const int64_t *d_out_off, int64_t n_rec, int32_t *d_batch,
-           uint8_t *d_mask, cudaStream_t st) {
+           uint8_t *d_mask, cudaStream_t st, int64_t ids_cap = INT64_MAX) {
     if (n_rec == 0) return DNATOK_OK;
     PadArgs a;
     a.ids = d_ids; a.out_off = d_out_off; a.n_rows = n_rec; a.batch_ids = d_batch; a.mask = d_mask;
     a.seq_len = h->cfg.seq_len; a.pad_side = h->cfg.pad_side; a.pad_id = h->cfg.pad_id;
+    a.ids_cap = ids_cap;
     int grid = (int)std::min<int64_t>(n_rec, (int64_t)h->sm_count * 16);
     if (h->grid_cap > 0) grid = std::min(grid, h->grid_cap);
     if (h->cfg.id_dtype == DNATOK_I16) pad_rows_kernel<int16_t><<<grid, 256, 0, st>>>(a);
@@ -391,6 +407,8 @@ void ring_free(StreamRing &r) {
         ctx_free(s.ctx);
     }
     for (auto st : r.streams) cudaStreamDestroy(st);
+    for (auto p : r.stage) cudaFreeHost(p);
+    for (auto e : r.ev_stage) if (e) cudaEventDestroy(e);
     r = StreamRing();
 }
 
@@ -422,6 +440,18 @@ int ring_setup(dnatok_t *h, int64_t chunk_bytes, int n_streams, int64_t max_rows
         CU(cudaEventCreateWithFlags(&s.ev_done, cudaEventDisableTiming));
         CU(cudaEventCreateWithFlags(&s.ev_off, cudaEventDisableTiming));
         int rc = ctx_init(h, s.ctx); if (rc) return rc;
+    }
+    return DNATOK_OK;
+}
+
+int ring_stage_setup(dnatok_t *h) {
+    StreamRing &r = h->ring;
+    if (!r.stage.empty()) return DNATOK_OK;
+    const int n = r.n_streams + 1;
+    r.stage.assign(n, nullptr); r.ev_stage.assign(n, nullptr);
+    for (int i = 0; i < n; ++i) {
+        CU(cudaHostAlloc((void **)&r.stage[i], (size_t)r.chunk_bytes, cudaHostAllocDefault));
+        CU(cudaEventCreateWithFlags(&r.ev_stage[i], cudaEventDisableTiming));
     }
     return DNATOK_OK;
 }
@@ -509,7 +539,8 @@ int dnatok_create(const dnatok_config *cfg_in, int device, dnatok_t **out) {
     if (!h) return DNATOK_ENOMEM;
     h->cfg = cfg; h->cfg.merges = nullptr; h->cfg.kmer_lut = nullptr; h->device = device;
     auto bail = [&](int code) { dnatok_destroy(h); return code; };
-    if (cudaSetDevice(device) != cudaSuccess) return bail(DNATOK_ECUDA);
+    DeviceGuard dev_guard_(device);
+    if (!dev_guard_.ok) return bail(DNATOK_ECUDA);
     cudaDeviceProp prop;
     if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) return bail(DNATOK_ECUDA);
     h->sm_count = prop.multiProcessorCount;
@@ -631,7 +662,7 @@ int dnatok_create(const dnatok_config *cfg_in, int device, dnatok_t **out) {
 
 int dnatok_destroy(dnatok_t *h) {
     if (!h) return DNATOK_OK;
-    cudaSetDevice(h->device);
+    DeviceGuard dev_guard_(h->device);
     cudaDeviceSynchronize();
     ring_free(h->ring);
     ctx_free(h->ctx);
@@ -646,7 +677,7 @@ int dnatok_encode(dnatok_t *h, const uint8_t *d_bytes, int64_t n_bytes, const in
     if (n_bytes < 0 || n_records < 0 || ids_capacity < 0 || !d_rec_offsets || !d_out_offsets ||
         (n_bytes > 0 && !d_bytes) || (ids_capacity > 0 && !d_ids_out))
         return fail(h, DNATOK_EINVAL, "dnatok_encode: bad argument");
-    CU(cudaSetDevice(h->device));
+    USE_DEVICE(h);
     return encode_on(h, h->ctx, d_bytes, n_bytes, d_rec_offsets, n_records, 0, d_ids_out, ids_capacity,
                      d_out_offsets, (cudaStream_t)stream);
 }
@@ -657,33 +688,21 @@ int dnatok_pad(dnatok_t *h, const void *d_ids, const int64_t *d_out_offsets, int
     if (h->cfg.seq_len <= 0) return fail(h, DNATOK_EINVAL, "dnatok_pad: handle was created with seq_len == 0");
     if (n_records < 0 || !d_out_offsets || (n_records > 0 && !d_batch_ids))
         return fail(h, DNATOK_EINVAL, "dnatok_pad: bad argument");
-    CU(cudaSetDevice(h->device));
+    USE_DEVICE(h);
     return pad_on(h, d_ids, d_out_offsets, n_records, d_batch_ids, d_mask, (cudaStream_t)stream);
 }
 
-int dnatok_stream_encode(dnatok_t *h, const uint8_t *h_pinned, int64_t n_bytes, const int64_t *h_rec_offsets,
-                         int64_t n_records, int64_t chunk_bytes, int n_streams, int64_t max_rows_per_chunk,
-                         dnatok_batch_fn on_batch, void *user) {
-    if (!h) return DNATOK_EINVAL;
-    if (n_bytes < 0 || n_records < 0 || !h_rec_offsets || chunk_bytes <= 0 || n_streams < 1 || n_streams > 64 ||
-        (n_bytes > 0 && !h_pinned))
-        return fail(h, DNATOK_EINVAL, "dnatok_stream_encode: bad argument");
-    CU(cudaSetDevice(h->device));
-    if (n_bytes > 0) {
-        cudaPointerAttributes at;
-        cudaError_t e = cudaPointerGetAttributes(&at, h_pinned);
-        if (e != cudaSuccess || at.type != cudaMemoryTypeHost) {
-            cudaGetLastError();
-            return fail(h, DNATOK_EINVAL, "dnatok_stream_encode: h_pinned is not page-locked host memory");
-        }
-    }
-    if (max_rows_per_chunk <= 0) max_rows_per_chunk = chunk_bytes / 64 + 2;
-    int rc = ring_setup(h, chunk_bytes, n_streams, max_rows_per_chunk);
-    if (rc) return rc;
+// The chunk loop of step 7.  h_pinned != NULL: the ring's host slots alias the caller's page-locked buffer.  Otherwise every
+// chunk is produced by fill(fill_user, chunk_index, offset, n_bytes, dst) into one of n_streams + 1 pinned staging slots
+// (PAPER.md:181 persistent pinned buffers) and copied to the device from there.  Any failure returns at once; the caller
+// drains the streams.
+static int stream_run(dnatok_t *h, const uint8_t *h_pinned, dnatok_fill_fn fill, void *fill_user, int64_t n_bytes,
+                      const int64_t *h_rec_offsets, int64_t n_records, dnatok_batch_fn on_batch, void *user) {
     StreamRing &R = h->ring;
-    const int64_t C = chunk_bytes;
+    const int64_t C = R.chunk_bytes;
     const int64_t n_chunks = std::max<int64_t>(1, (n_bytes + C - 1) / C);
-    const size_t idsz = (size_t)h->cfg.id_dtype;
+    const int n_stage = (int)R.stage.size();
+    int rc;
     int64_t ra = 0;                                   // first record not yet delivered
     for (int64_t i = 0; i < n_chunks; ++i) {
         StreamSlot &S = R.slots[i % R.n_slots];
@@ -695,18 +714,23 @@ int dnatok_stream_encode(dnatok_t *h, const uint8_t *h_pinned, int64_t n_bytes, 
         else rb = std::upper_bound(h_rec_offsets + ra + 1, h_rec_offsets + n_records + 1, c1) - h_rec_offsets - 1;
         if (rb < ra) rb = ra;
         const int64_t rows = rb - ra;
-        if (rows > R.max_rows) {
-            for (auto s2 : R.streams) cudaStreamSynchronize(s2);
+        if (rows > R.max_rows)
             return fail(h, DNATOK_ECAPACITY, "chunk %lld holds %lld records > max_rows_per_chunk %lld",
                         (long long)i, (long long)rows, (long long)R.max_rows);
-        }
         // bytes of the record cut by the previous boundary live in the previous slot's buffer
         const int64_t data0 = std::min(h_rec_offsets[ra], c0);       // host offset of the first byte needed
         const int64_t carry = c0 - data0;
-        if (carry > R.carry_cap) {
-            for (auto s2 : R.streams) cudaStreamSynchronize(s2);
+        if (carry > R.carry_cap)
             return fail(h, DNATOK_ECAPACITY, "record %lld needs %lld carried bytes > max_record_bytes %lld",
                         (long long)ra, (long long)carry, (long long)R.carry_cap);
+        // the producer fills its staging slot while earlier chunks are still in flight
+        const uint8_t *src = h_pinned ? h_pinned + c0 : nullptr;
+        if (!h_pinned && c1 > c0) {
+            const int sl = (int)(i % n_stage);
+            CU(cudaEventSynchronize(R.ev_stage[sl]));                 // the copy out of its previous use has finished
+            if (fill(fill_user, i, c0, c1 - c0, R.stage[sl]) != 0)
+                return fail(h, DNATOK_EINVAL, "dnatok_stream_encode_from: the producer failed on chunk %lld", (long long)i);
+            src = R.stage[sl];
         }
         uint8_t *d_chunk = S.d_buf + R.carry_cap;
         // this buffer was last used by chunk i - n_slots (same stream only if n_slots == n_streams) and read by
@@ -722,8 +746,9 @@ int dnatok_stream_encode(dnatok_t *h, const uint8_t *h_pinned, int64_t n_bytes, 
                                cudaMemcpyDeviceToDevice, st));
         }
         CU(cudaEventRecord(S.ev_carry, st));
-        if (c1 > c0) CU(cudaMemcpyAsync(d_chunk, h_pinned + c0, (size_t)(c1 - c0), cudaMemcpyHostToDevice, st));
+        if (c1 > c0) CU(cudaMemcpyAsync(d_chunk, src, (size_t)(c1 - c0), cudaMemcpyHostToDevice, st));
         CU(cudaEventRecord(S.ev_h2d, st));
+        if (!h_pinned && c1 > c0) CU(cudaEventRecord(R.ev_stage[i % n_stage], st));
         // record offsets of this batch (staged through the slot's pinned buffer)
         CU(cudaEventSynchronize(S.ev_off));
         memcpy(S.h_recoff, h_rec_offsets + ra, (size_t)(rows + 1) * sizeof(int64_t));
@@ -735,7 +760,7 @@ int dnatok_stream_encode(dnatok_t *h, const uint8_t *h_pinned, int64_t n_bytes, 
                        S.d_out_off, st);
         if (rc) return rc;
         if (h->cfg.seq_len > 0) {
-            rc = pad_on(h, S.d_ids, S.d_out_off, rows, S.d_batch, S.d_mask, st);
+            rc = pad_on(h, S.d_ids, S.d_out_off, rows, S.d_batch, S.d_mask, st, R.carry_cap + C);
             if (rc) return rc;
         }
         if (on_batch) {
@@ -749,15 +774,67 @@ int dnatok_stream_encode(dnatok_t *h, const uint8_t *h_pinned, int64_t n_bytes, 
         CU(cudaEventRecord(S.ev_done, st));
         ra = rb;
     }
-    (void)idsz;
     for (auto st : R.streams) CU(cudaStreamSynchronize(st));
-    for (auto &s : R.slots) { rc = status_of(h, s.ctx); if (rc) return rc; }
+    for (auto &sl : R.slots) { rc = status_of(h, sl.ctx); if (rc) return rc; }
     return DNATOK_OK;
+}
+
+static int stream_entry(dnatok_t *h, const uint8_t *h_pinned, dnatok_fill_fn fill, void *fill_user, int64_t n_bytes,
+                        const int64_t *h_rec_offsets, int64_t n_records, int64_t chunk_bytes, int n_streams,
+                        int64_t max_rows_per_chunk, dnatok_batch_fn on_batch, void *user) {
+    if (max_rows_per_chunk <= 0) max_rows_per_chunk = chunk_bytes / 64 + 2;
+    int rc = ring_setup(h, chunk_bytes, n_streams, max_rows_per_chunk);
+    if (rc == DNATOK_OK && !h_pinned) rc = ring_stage_setup(h);
+    if (rc == DNATOK_OK) rc = stream_run(h, h_pinned, fill, fill_user, n_bytes, h_rec_offsets, n_records, on_batch, user);
+    if (rc != DNATOK_OK) {
+        // nothing stays in flight behind a failed call: the ring's streams are drained and a sticky CUDA error is cleared
+        for (auto st : h->ring.streams) cudaStreamSynchronize(st);
+        cudaGetLastError();
+    }
+    return rc;
+}
+
+static int fill_from_memory(void *user, int64_t, int64_t offset, int64_t n, uint8_t *dst) {
+    memcpy(dst, static_cast<const uint8_t *>(user) + offset, (size_t)n);
+    return 0;
+}
+
+int dnatok_stream_encode(dnatok_t *h, const uint8_t *h_bytes, int64_t n_bytes, const int64_t *h_rec_offsets,
+                         int64_t n_records, int64_t chunk_bytes, int n_streams, int64_t max_rows_per_chunk,
+                         dnatok_batch_fn on_batch, void *user) {
+    if (!h) return DNATOK_EINVAL;
+    if (n_bytes < 0 || n_records < 0 || !h_rec_offsets || chunk_bytes <= 0 || n_streams < 1 || n_streams > 64 ||
+        (n_bytes > 0 && !h_bytes))
+        return fail(h, DNATOK_EINVAL, "dnatok_stream_encode: bad argument");
+    USE_DEVICE(h);
+    bool pinned = n_bytes == 0;
+    if (n_bytes > 0) {
+        cudaPointerAttributes at;
+        cudaError_t e = cudaPointerGetAttributes(&at, h_bytes);
+        if (e != cudaSuccess) cudaGetLastError();
+        else if (at.type == cudaMemoryTypeDevice || at.type == cudaMemoryTypeManaged)
+            return fail(h, DNATOK_EINVAL, "dnatok_stream_encode: h_bytes is not host memory");
+        pinned = e == cudaSuccess && at.type == cudaMemoryTypeHost;
+    }
+    // page-locked input: the ring's host slots alias it; pageable input goes through the pinned staging ring
+    return stream_entry(h, pinned ? h_bytes : nullptr, fill_from_memory, const_cast<uint8_t *>(h_bytes), n_bytes, h_rec_offsets,
+                        n_records, chunk_bytes, n_streams, max_rows_per_chunk, on_batch, user);
+}
+
+int dnatok_stream_encode_from(dnatok_t *h, dnatok_fill_fn fill, void *fill_user, int64_t n_bytes,
+                              const int64_t *h_rec_offsets, int64_t n_records, int64_t chunk_bytes, int n_streams,
+                              int64_t max_rows_per_chunk, dnatok_batch_fn on_batch, void *user) {
+    if (!h) return DNATOK_EINVAL;
+    if (!fill || n_bytes < 0 || n_records < 0 || !h_rec_offsets || chunk_bytes <= 0 || n_streams < 1 || n_streams > 64)
+        return fail(h, DNATOK_EINVAL, "dnatok_stream_encode_from: bad argument");
+    USE_DEVICE(h);
+    return stream_entry(h, nullptr, fill, fill_user, n_bytes, h_rec_offsets, n_records, chunk_bytes, n_streams,
+                        max_rows_per_chunk, on_batch, user);
 }
 
 int dnatok_check(dnatok_t *h, void *stream) {
     if (!h) return DNATOK_EINVAL;
-    CU(cudaSetDevice(h->device));
+    USE_DEVICE(h);
     CU(cudaStreamSynchronize((cudaStream_t)stream));
     return status_of(h, h->ctx);
 }
@@ -795,7 +872,7 @@ int dnatok_revcomp(dnatok_t *h, const uint8_t *d_bytes, int64_t n_bytes, const i
     if (n_bytes < 0 || n_records < 0 || !d_rec_offsets || (n_bytes > 0 && (!d_bytes || !d_out)) || d_bytes == d_out)
         return fail(h, DNATOK_EINVAL, "dnatok_revcomp: bad argument (in-place is not supported)");
     if (n_bytes == 0) return DNATOK_OK;
-    CU(cudaSetDevice(h->device));
+    USE_DEVICE(h);
     RevcompArgs a{d_bytes, d_out, d_rec_offsets, n_records, n_bytes};
     const int64_t n16 = (n_bytes + 15) >> 4;
     int grid = (int)std::min<int64_t>((n16 + 255) / 256, (int64_t)h->sm_count * 8);
@@ -814,7 +891,7 @@ int dnatok_decode(dnatok_t *h, const void *d_ids, const int64_t *d_out_offsets, 
     if (h->d_remap4) return fail(h, DNATOK_EINVAL, "dnatok_decode: a handle with a k-mer id table has no inverse table");
     if (h->cfg.mode == DNATOK_BPE && !h->d_spell)
         return fail(h, DNATOK_EINVAL, "dnatok_decode: the merge table's token spellings exceed 64 MiB");
-    CU(cudaSetDevice(h->device));
+    USE_DEVICE(h);
     cudaStream_t st = (cudaStream_t)stream;
     if (n_records + 1 > h->rec_len_cap) {
         if (h->d_rec_len) CU(cudaFreeAsync(h->d_rec_len, st));
@@ -857,7 +934,7 @@ int dnatok_embed(dnatok_t *h, const int32_t *d_ids, int64_t n_rows, int64_t t_le
         row_bytes > (1 << 20) || (n_rows > 0 && (!d_ids || !d_table || !d_out)) ||
         (reinterpret_cast<uintptr_t>(d_table) & 3) || (reinterpret_cast<uintptr_t>(d_out) & 3))
         return fail(h, DNATOK_EINVAL, "dnatok_embed: bad argument (row_bytes must be a multiple of 4, buffers 4-byte aligned)");
-    CU(cudaSetDevice(h->device));
+    USE_DEVICE(h);
     const bool v16 = (row_bytes & 15) == 0 && (reinterpret_cast<uintptr_t>(d_table) & 15) == 0 &&
                      (reinterpret_cast<uintptr_t>(d_out) & 15) == 0;
     const int64_t b = dnatok_microbatch_rows(b_emb, m_tokens, t_len);
@@ -880,7 +957,7 @@ int dnatok_widen_ids(dnatok_t *h, const int32_t *d_ids, int64_t n, int64_t *d_ou
     if (!h) return DNATOK_EINVAL;
     if (n < 0 || (n > 0 && (!d_ids || !d_out))) return fail(h, DNATOK_EINVAL, "dnatok_widen_ids: bad argument");
     if (n == 0) return DNATOK_OK;
-    CU(cudaSetDevice(h->device));
+    USE_DEVICE(h);
     int grid = (int)std::min<int64_t>((n / 4 + 255) / 256 + 1, (int64_t)h->sm_count * 8);
     if (h->grid_cap > 0) grid = std::min(grid, h->grid_cap);
     widen_kernel<<<grid, 256, 0, (cudaStream_t)stream>>>(d_ids, n, d_out);

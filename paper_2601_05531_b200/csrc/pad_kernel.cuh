@@ -17,6 +17,7 @@ struct PadArgs {
     int32_t *batch_ids;
     uint8_t *mask;              // may be null
     int32_t seq_len, pad_side, pad_id;
+    int64_t ids_cap;            // ids beyond it were never written (an encode that overflowed): read as pad_id
 };
 
 // one CTA per row (grid-stride), each thread writes 4 consecutive columns per step
@@ -24,7 +25,9 @@ template <typename IdT>
 __global__ void __launch_bounds__(256) pad_rows_kernel(const __grid_constant__ PadArgs A) {
     const IdT *ids = reinterpret_cast<const IdT *>(A.ids);
     const int L = A.seq_len;
-    const bool vec = (L & 3) == 0;
+    // 16-byte id stores and 4-byte mask stores need aligned rows: seq_len a multiple of 4 and aligned base pointers
+    const bool vec = (L & 3) == 0 && (reinterpret_cast<uintptr_t>(A.batch_ids) & 15) == 0 &&
+                     (reinterpret_cast<uintptr_t>(A.mask) & 3) == 0;
     for (int64_t r = blockIdx.x; r < A.n_rows; r += gridDim.x) {
         const int64_t o0 = A.out_off[r];
         const int64_t tok = A.out_off[r + 1] - o0;
@@ -40,7 +43,7 @@ __global__ void __launch_bounds__(256) pad_rows_kernel(const __grid_constant__ P
                 for (int j = 0; j < 4; ++j) {
                     int q = c + j - col0;
                     bool in = q >= 0 && q < m;
-                    pv[j] = in ? (int32_t)ids[o0 + q] : A.pad_id;
+                    pv[j] = (in && o0 + q < A.ids_cap) ? (int32_t)ids[o0 + q] : A.pad_id;
                     mk |= (uint32_t)in << (8 * j);
                 }
                 *reinterpret_cast<int4 *>(row + c) = v;
@@ -50,7 +53,7 @@ __global__ void __launch_bounds__(256) pad_rows_kernel(const __grid_constant__ P
             for (int c = threadIdx.x; c < L; c += blockDim.x) {
                 int q = c - col0;
                 bool in = q >= 0 && q < m;
-                row[c] = in ? (int32_t)ids[o0 + q] : A.pad_id;
+                row[c] = (in && o0 + q < A.ids_cap) ? (int32_t)ids[o0 + q] : A.pad_id;
                 if (mrow) mrow[c] = in ? 1 : 0;
             }
         }

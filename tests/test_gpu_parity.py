@@ -389,3 +389,69 @@ def test_pad_handworked(golden_dir):
         batch, mask = tok.encode_padded(torch.from_numpy(data).cuda(), torch.tensor(g["rec_offsets"]).cuda())
         tok.check()
         assert batch.cpu().tolist() == g[key]["ids"] and mask.cpu().tolist() == g[key]["mask"]
+
+
+# ------------------------------------------------------------------------------------------- custom tables on every path
+def _lut(**over):
+    lut = oracle.default_lut()
+    for ch, c in over.items():
+        lut[ord(ch)] = c
+    return lut
+
+
+@pytest.mark.parametrize("name,lut", [
+    ("soft-masked lowercase is N (no arithmetic classification of acgt)", dict(a=4, c=4, g=4, t=4)),
+    ("N is UNK (runs of N take the table)", dict(N=5, n=5)),
+    ("'-' and '*' are skipped, 'U' is T", {"-": 255, "*": 255, "U": 3, "u": 3}),
+    ("'>' itself is a SKIP byte but still opens a header", {">": 255}),
+])
+@pytest.mark.parametrize("k", [1, 6])
+def test_custom_luts_on_multi_super_tile_fasta(name, lut, k):
+    """EncParams.fast_lut = 0 / fast_n = 0 and extra SKIP bytes, on FASTA that spans many super-tiles, with headers and skipped
+    bytes sprinkled around the super-tile edges (16 KiB multiples)"""
+    w = dnagen.config3(total_bases=600_000, lo=1000, hi=70_000, seed=5)
+    data = w.data.copy()
+    rng = np.random.default_rng(k)
+    edges = np.arange(16384, data.size - 200, 16384)
+    for e in edges:                                           # soft-masked runs, gaps and stops around every edge
+        a = int(e + rng.integers(-150, 150))
+        run = data[a: a + 40]
+        keep = run != 10
+        if rng.random() < 0.5:
+            run[keep] = np.char.lower(run[keep].view("S1")).view(np.uint8)
+        else:
+            run[keep & (rng.random(40) < 0.3)] = ord("-")
+        data[int(e + rng.integers(-3, 3))] = rng.choice(np.frombuffer(b"*-Nn>U", dtype=np.uint8))
+    data[data == 0] = ord("A")
+    check(data, w.offsets, mode="kmer", k=k, class_lut=_lut(**lut))
+
+
+@pytest.mark.parametrize("mode,k,dt", [("single_nt", 1, 4), ("kmer", 6, 2), ("kmer", 3, 4)])
+def test_ids_out_pointer_that_is_not_16_byte_aligned(mode, k, dt):
+    w = dnagen.config3(total_bases=200_000, lo=100, hi=30_000)
+    kw = dict(mode=mode, k=k, id_dtype=dt)
+    tok = dn.DNATok(**kw)
+    d, o = torch.from_numpy(w.data).cuda(), torch.from_numpy(w.offsets).cuda()
+    buf = torch.empty(w.data.size + 8, dtype=tok.id_torch_dtype, device="cuda")
+    want_ids, want_off = oracle.encode(w.data, w.offsets, ocfg(**kw))
+    for shift in (1, 3):
+        ids, out = tok.encode(d, o, ids_out=buf[shift:])
+        tok.check()
+        out = out.cpu().numpy()
+        assert np.array_equal(out, want_off) and np.array_equal(ids[: out[-1]].cpu().numpy().astype(np.int32), want_ids)
+
+
+def test_pad_into_unaligned_views():
+    w = dnagen.config3(total_bases=60_000, lo=10, hi=3000)
+    tok = dn.DNATok(mode="kmer", k=6, seq_len=64)
+    d, o = torch.from_numpy(w.data).cuda(), torch.from_numpy(w.offsets).cuda()
+    ids, out = tok.encode(d, o)
+    n = w.n_records
+    bbuf = torch.empty(n * 64 + 4, dtype=torch.int32, device="cuda")
+    mbuf = torch.empty(n * 64 + 4, dtype=torch.uint8, device="cuda")
+    batch, mask = tok.pad(ids, out, batch_ids=bbuf[1: 1 + n * 64].view(n, 64), mask=mbuf[1: 1 + n * 64].view(n, 64))
+    tok.check()
+    c = oracle.Config(mode=oracle.KMER, k=6, seq_len=64)
+    wi, wo = oracle.encode(w.data, w.offsets, c)
+    wb, wm = oracle.pad(wi, wo, c)
+    assert np.array_equal(batch.cpu().numpy(), wb) and np.array_equal(mask.cpu().numpy(), wm)

@@ -14,9 +14,9 @@ if torch.cuda.is_available():
     import paper_2601_05531_b200 as dn
 
 
-def run_stream(w, chunk_bytes, n_streams, **kw):
+def run_stream(w, chunk_bytes, n_streams, source="pinned", **kw):
     tok = dn.DNATok(**kw)
-    pinned = torch.from_numpy(w.data.copy()).pin_memory()
+    pinned = torch.from_numpy(w.data.copy()).pin_memory() if source == "pinned" else w.data.copy()   # pageable numpy array
     got_ids, got_cnt, got_batch, got_mask, firsts = [], [], [], [], []
     keep = []
 
@@ -32,7 +32,18 @@ def run_stream(w, chunk_bytes, n_streams, **kw):
                 got_mask.append(b.mask().cpu().numpy())
             firsts.append((b.first_record, b.n_records))
 
-    tok.stream_encode(pinned, w.offsets, chunk_bytes, n_streams, max_rows_per_chunk=w.n_records + 1, on_batch=on_batch)
+    if source == "file":
+        import tempfile
+        with tempfile.NamedTemporaryFile() as f:
+            f.write(w.data.tobytes()); f.flush()
+            with open(f.name, "rb", buffering=0) as rd:
+                def fill(i, off, dst):
+                    rd.seek(off)
+                    assert rd.readinto(dst) == dst.size
+                tok.stream_encode_from(fill, w.data.size, w.offsets, chunk_bytes, n_streams, max_rows_per_chunk=w.n_records + 1,
+                                       on_batch=on_batch)
+    else:
+        tok.stream_encode(pinned, w.offsets, chunk_bytes, n_streams, max_rows_per_chunk=w.n_records + 1, on_batch=on_batch)
     # batches arrive in record order and cover every record exactly once
     pos = 0
     for f, n in firsts:
@@ -92,12 +103,54 @@ def test_stream_bpe():
     assert np.array_equal(got[0], want[0]) and np.array_equal(got[1], want[1])
 
 
-def test_carry_capacity_error_and_unpinned_rejected():
+def test_carry_capacity_error_and_device_pointer_rejected():
     w = dnagen.config3(total_bases=100_000, lo=50_000, hi=100_000)
     tok = dn.DNATok(mode="kmer", k=6, max_record_bytes=1024)
     with pytest.raises(dn.DNATokError) as e:
         tok.stream_encode(torch.from_numpy(w.data.copy()).pin_memory(), w.offsets, 8192, 2)
     assert e.value.code == dn.ECAPACITY
+    with pytest.raises(dn.DNATokError) as e:                              # a device pointer is not host memory
+        dn.dnatok_stream_encode(tok.h, torch.from_numpy(w.data.copy()).cuda().data_ptr(), w.data.size, w.offsets.ctypes.data,
+                                w.n_records, 8192, 2, 0, dn._BATCH_FN(lambda *_: None))
+    assert e.value.code == dn.EINVAL
+
+
+@pytest.mark.parametrize("source", ["pageable", "file"])
+@pytest.mark.parametrize("chunk_bytes,n_streams", [(4099, 1), (65536 + 7, 4), (1 << 20, 2)])
+def test_pageable_and_file_input_go_through_the_pinned_staging_ring(source, chunk_bytes, n_streams):
+    """a producer reading from a file or pageable memory fills a ring of n_streams + 1 pinned slots
+    (PAPER.md:181 persistent pinned buffers); the result is the whole-buffer result"""
+    w = dnagen.config3(total_bases=300_000, lo=1000, hi=20000)
+    kw = dict(mode="kmer", k=6, seq_len=512, max_record_bytes=32768)
+    want = oracle_ref(w, **kw)
+    got = run_stream(w, chunk_bytes, n_streams, source=source, **kw)
+    for g, x in zip(got, want):
+        assert np.array_equal(g, x)
+
+
+def test_failed_stream_call_leaves_nothing_in_flight_and_the_handle_usable():
+    """a capacity failure in the middle of the chunk loop (a record longer than the carry buffer) drains the ring; the next
+    call on the same handle works; a failing producer is reported as EINVAL"""
+    w = dnagen.config3(total_bases=300_000, lo=50_000, hi=131072)
+    tok = dn.DNATok(mode="kmer", k=6, max_record_bytes=4096)
+    pinned = torch.from_numpy(w.data.copy()).pin_memory()
     with pytest.raises(dn.DNATokError) as e:
-        tok.stream_encode(torch.from_numpy(w.data.copy()), w.offsets, 8192, 2)
+        tok.stream_encode(pinned, w.offsets, 16384, 4, max_rows_per_chunk=64)
+    assert e.value.code == dn.ECAPACITY
+    torch.cuda.synchronize()
+    small = dnagen.config3(total_bases=50_000, lo=100, hi=2000)
+    cnt = []
+
+    def on_batch(b):
+        with torch.cuda.stream(torch.cuda.ExternalStream(b.stream)):      # read on the batch's own stream
+            cnt.append(np.diff(b.out_offsets().cpu().numpy()))
+    tok.stream_encode(torch.from_numpy(small.data.copy()).pin_memory(), small.offsets, 16384, 4, max_rows_per_chunk=small.n_records + 1,
+                      on_batch=on_batch)
+    _, want_off = oracle.encode(small.data, small.offsets, oracle.Config(mode=oracle.KMER, k=6))
+    assert np.array_equal(np.concatenate(cnt), np.diff(want_off))
+
+    def bad_fill(i, off, dst):
+        raise IOError("no such chunk")
+    with pytest.raises(dn.DNATokError) as e:
+        tok.stream_encode_from(bad_fill, small.data.size, small.offsets, 16384, 2)
     assert e.value.code == dn.EINVAL
