@@ -412,7 +412,7 @@ def bench_config(dn, torch, D: Dist, local: int, config: int, k: int, args, *, e
     clk = clocks.stop()
     tok.check()
     ms_per_step = D.max(total_ms / args.steps)
-    assert launches >= 2 * args.steps, "the CUDA library launched no kernels: there is no CPU path"
+    assert launches >= args.steps, "the CUDA library launched no kernels: there is no CPU path"
 
     # ---- parity against the oracle (untimed): every offset, the ids of sampled records ------------------------------
     parity_s = "skipped"

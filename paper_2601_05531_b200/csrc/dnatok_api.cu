@@ -264,9 +264,14 @@ int launch_tiles(dnatok_t *h, EncCtx &c, const EncParams &prm, const uint8_t *d_
         h->launches += 1;
         launch_dense<IdT>(a, kk, grid, st);
     } else {
-        v5::tile_first_rec_kernel<<<nb_first, 256, 0, st>>>(a);
-        CU(cudaGetLastError());
-        h->launches += 1;
+        // an input that gives every CTA at most one tile is encoded in ONE launch: the record range of a tile is searched
+        // inside the kernel instead of by the pre-pass (SURVEY.md section 7 hard part 6)
+        if (n_tiles <= slots && n_rec <= (1 << 16)) a.first_rec = nullptr;
+        else {
+            v5::tile_first_rec_kernel<<<nb_first, 256, 0, st>>>(a);
+            CU(cudaGetLastError());
+            h->launches += 1;
+        }
         launch_strip<IdT>(a, kk, grid, st);
     }
     CU(cudaGetLastError());

@@ -502,7 +502,21 @@ __device__ __forceinline__ void prep_super(const EncArgs &A, Smem5 &sm, int par,
     }
     const int64_t t0n = (int64_t)tile_n * A.S * TB;
     if (lane < 2 && lane < A.S) prefetch_l2(A, t0n + (int64_t)lane * TB);
-    const int64_t rlo = A.first_rec[tile_n], rhi = A.first_rec[tile_n + 1];
+    int64_t rlo, rhi;
+    if (A.first_rec) { rlo = A.first_rec[tile_n]; rhi = A.first_rec[tile_n + 1]; }
+    else {
+        // small inputs run without the pre-pass launch: lanes 0 and 1 search rec_offsets for this tile and the next one
+        int64_t lo = 0, hi = A.n_rec + 1;
+        const int64_t tt = (int64_t)tile_n + (lane & 1);
+        if (tt < A.n_tiles) {
+            const int64_t pos = tt * A.S * TB;
+            while (lo < hi) {
+                const int64_t mid = (lo + hi) >> 1;
+                if (rec_pos(A, mid) >= pos) hi = mid; else lo = mid + 1;
+            }
+        } else lo = A.n_rec + 1;
+        rlo = __shfl_sync(FULL, lo, 0); rhi = __shfl_sync(FULL, lo, 1);
+    }
     const int64_t m64 = rhi - rlo;
     const int m = m64 > 0x7fffffff ? 0x7fffffff : (int)m64;
     if (m <= EVW && lane < m) sm.ev_p[par][lane] = (int)(rec_pos(A, rlo + lane) - t0n);
