@@ -454,7 +454,7 @@ def bench_config(dn, torch, D: Dist, local: int, config: int, k: int, args, *, e
         out_bytes = n_tokens * idsz + (n_rec + 1) * 8
     alg_bytes = in_bytes + out_bytes
     kern_ms = float(np.median(per_step_ms))
-    kname = {"bpe": "bpe_segments_kernel"}.get(tokkw["mode"], "encode_tiles_v7<dense>" if tok.cfg.class_lut is not None
+    kname = {"bpe": "bpe_merge_kernel"}.get(tokkw["mode"], "encode_tiles_v7<dense>" if tok.cfg.class_lut is not None
                                                and not tok.cfg.strip_headers else "encode_tiles_v5")
     roof = {"bound": "hbm", "kernel": kname, "achieved": alg_bytes / (kern_ms * 1e-3) / 1e9, "peak": peak, "unit": "GB/s",
             "peak_source": peak_src, "algorithmic_bytes_per_launch": alg_bytes,
