@@ -1,7 +1,8 @@
 """Build libdnatok.so (the C-ABI shared library) in-tree with nvcc for sm_100a.
 
 nvcc cross-compiles without a GPU; the built .so is git-ignored but travels to the GPU box with the
-gpurun snapshot.  `python -m paper_2601_05531_b200._build [--force] [--verbose]`.
+gpurun snapshot.  `python -m paper_2601_05531_b200._build [--force] [--verbose]`; extra nvcc flags for debug builds
+come from the environment variable DTK_NVCC_FLAGS (e.g. -DDTK_PROF for the phase timers).
 """
 from __future__ import annotations
 
@@ -38,7 +39,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
     if not force and not stale():
         return LIB
     tmp = LIB + f".tmp{os.getpid()}"
-    cmd = [NVCC, *FLAGS, *(["-Xptxas", "-v"] if verbose else []), "-o", tmp, *sources()]
+    cmd = [NVCC, *FLAGS, *os.environ.get("DTK_NVCC_FLAGS", "").split(), *(["-Xptxas", "-v"] if verbose else []), "-o", tmp, *sources()]
     if verbose:
         print(" ".join(cmd), flush=True)
     subprocess.check_call(cmd)

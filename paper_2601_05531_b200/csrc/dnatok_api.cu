@@ -191,20 +191,33 @@ int ctx_next_gen(dnatok_t *h, EncCtx &c, cudaStream_t st) {
     return DNATOK_OK;
 }
 
+// launch of an encode kernel behind its pre-pass with programmatic stream serialisation (the kernel's prologue overlaps
+// the pre-pass's tail; the kernel waits with griddepcontrol.wait before it reads what the pre-pass wrote)
+template <typename K>
+void launch_pdl(K kernel, int grid, int block, size_t smem, cudaStream_t st, const EncArgs &a, bool pdl) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)grid); cfg.blockDim = dim3((unsigned)block); cfg.dynamicSmemBytes = smem; cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr; cfg.numAttrs = pdl ? 1 : 0;
+    cudaLaunchKernelEx(&cfg, kernel, a);
+}
+
 // the headline shapes get a kernel with only their own emission variant compiled in (smaller instruction footprint)
 template <typename IdT>
 void launch_dense(const EncArgs &a, int kk, int grid, cudaStream_t st) {
     constexpr bool wide = sizeof(IdT) >= 2;                    // uint8 ids: the BPE class pass, single-nt only
     switch (wide ? kk : 0) {
-        case 0: v7::encode_tiles_v7<IdT, 0, true><<<grid, v7::NT7, sizeof(v7::Smem7), st>>>(a); break;
-        case 1: v7::encode_tiles_v7<IdT, wide ? 1 : 0, true><<<grid, v7::NT7, sizeof(v7::Smem7), st>>>(a); break;
-        case 2: v7::encode_tiles_v7<IdT, wide ? 2 : 0, true><<<grid, v7::NT7, sizeof(v7::Smem7), st>>>(a); break;
-        case 3: v7::encode_tiles_v7<IdT, wide ? 3 : 0, true><<<grid, v7::NT7, sizeof(v7::Smem7), st>>>(a); break;
-        case 4: v7::encode_tiles_v7<IdT, wide ? 4 : 0, true><<<grid, v7::NT7, sizeof(v7::Smem7), st>>>(a); break;
-        case 5: v7::encode_tiles_v7<IdT, wide ? 5 : 0, true><<<grid, v7::NT7, sizeof(v7::Smem7), st>>>(a); break;
-        case 6: v7::encode_tiles_v7<IdT, wide ? 6 : 0, true><<<grid, v7::NT7, sizeof(v7::Smem7), st>>>(a); break;
-        case 8: v7::encode_tiles_v7<IdT, wide ? 8 : 0, true><<<grid, v7::NT7, sizeof(v7::Smem7), st>>>(a); break;
-        default: v7::encode_tiles_v7<IdT, wide ? -1 : 0, true><<<grid, v7::NT7, sizeof(v7::Smem7), st>>>(a); break;
+        case 0: launch_pdl(v7::encode_tiles_v7<IdT, 0, true>, grid, v7::NT7, sizeof(v7::Smem7), st, a, true); break;
+        case 1: launch_pdl(v7::encode_tiles_v7<IdT, wide ? 1 : 0, true>, grid, v7::NT7, sizeof(v7::Smem7), st, a, true); break;
+        case 2: launch_pdl(v7::encode_tiles_v7<IdT, wide ? 2 : 0, true>, grid, v7::NT7, sizeof(v7::Smem7), st, a, true); break;
+        case 3: launch_pdl(v7::encode_tiles_v7<IdT, wide ? 3 : 0, true>, grid, v7::NT7, sizeof(v7::Smem7), st, a, true); break;
+        case 4: launch_pdl(v7::encode_tiles_v7<IdT, wide ? 4 : 0, true>, grid, v7::NT7, sizeof(v7::Smem7), st, a, true); break;
+        case 5: launch_pdl(v7::encode_tiles_v7<IdT, wide ? 5 : 0, true>, grid, v7::NT7, sizeof(v7::Smem7), st, a, true); break;
+        case 6: launch_pdl(v7::encode_tiles_v7<IdT, wide ? 6 : 0, true>, grid, v7::NT7, sizeof(v7::Smem7), st, a, true); break;
+        case 8: launch_pdl(v7::encode_tiles_v7<IdT, wide ? 8 : 0, true>, grid, v7::NT7, sizeof(v7::Smem7), st, a, true); break;
+        default: launch_pdl(v7::encode_tiles_v7<IdT, wide ? -1 : 0, true>, grid, v7::NT7, sizeof(v7::Smem7), st, a, true); break;
     }
 }
 template <typename IdT>
@@ -212,15 +225,15 @@ void launch_strip(const EncArgs &a, int kk, int grid, cudaStream_t st) {
     using namespace dtk::v5;
     constexpr bool wide = sizeof(IdT) >= 2;
     switch (wide ? kk : 0) {
-        case 0: encode_tiles_v5<IdT, 0><<<grid, NT, sizeof(Smem5), st>>>(a); break;
-        case 1: encode_tiles_v5<IdT, wide ? 1 : 0><<<grid, NT, sizeof(Smem5), st>>>(a); break;
-        case 2: encode_tiles_v5<IdT, wide ? 2 : 0><<<grid, NT, sizeof(Smem5), st>>>(a); break;
-        case 3: encode_tiles_v5<IdT, wide ? 3 : 0><<<grid, NT, sizeof(Smem5), st>>>(a); break;
-        case 4: encode_tiles_v5<IdT, wide ? 4 : 0><<<grid, NT, sizeof(Smem5), st>>>(a); break;
-        case 5: encode_tiles_v5<IdT, wide ? 5 : 0><<<grid, NT, sizeof(Smem5), st>>>(a); break;
-        case 6: encode_tiles_v5<IdT, wide ? 6 : 0><<<grid, NT, sizeof(Smem5), st>>>(a); break;
-        case 8: encode_tiles_v5<IdT, wide ? 8 : 0><<<grid, NT, sizeof(Smem5), st>>>(a); break;
-        default: encode_tiles_v5<IdT, wide ? -1 : 0><<<grid, NT, sizeof(Smem5), st>>>(a); break;
+        case 0: launch_pdl(encode_tiles_v5<IdT, 0>, grid, NT, sizeof(Smem5), st, a, a.first_rec != nullptr); break;
+        case 1: launch_pdl(encode_tiles_v5<IdT, wide ? 1 : 0>, grid, NT, sizeof(Smem5), st, a, a.first_rec != nullptr); break;
+        case 2: launch_pdl(encode_tiles_v5<IdT, wide ? 2 : 0>, grid, NT, sizeof(Smem5), st, a, a.first_rec != nullptr); break;
+        case 3: launch_pdl(encode_tiles_v5<IdT, wide ? 3 : 0>, grid, NT, sizeof(Smem5), st, a, a.first_rec != nullptr); break;
+        case 4: launch_pdl(encode_tiles_v5<IdT, wide ? 4 : 0>, grid, NT, sizeof(Smem5), st, a, a.first_rec != nullptr); break;
+        case 5: launch_pdl(encode_tiles_v5<IdT, wide ? 5 : 0>, grid, NT, sizeof(Smem5), st, a, a.first_rec != nullptr); break;
+        case 6: launch_pdl(encode_tiles_v5<IdT, wide ? 6 : 0>, grid, NT, sizeof(Smem5), st, a, a.first_rec != nullptr); break;
+        case 8: launch_pdl(encode_tiles_v5<IdT, wide ? 8 : 0>, grid, NT, sizeof(Smem5), st, a, a.first_rec != nullptr); break;
+        default: launch_pdl(encode_tiles_v5<IdT, wide ? -1 : 0>, grid, NT, sizeof(Smem5), st, a, a.first_rec != nullptr); break;
     }
 }
 

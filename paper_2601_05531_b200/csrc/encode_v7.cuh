@@ -474,6 +474,7 @@ __global__ void __launch_bounds__(DS_NT) dense_prepass_kernel(const __grid_const
     __shared__ long long wsum[DS_NT / 32];
     __shared__ long long s_base;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");   // the encode kernel may start its prologue now
     if ((int)blockIdx.x < nb_first) {
         const int64_t t = (int64_t)blockIdx.x * DS_NT + tid;
         if (t > A.n_tiles) return;

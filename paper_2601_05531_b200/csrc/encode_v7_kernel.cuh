@@ -27,6 +27,9 @@ __global__ void __launch_bounds__(NT7, 3) encode_tiles_v7(const __grid_constant_
     const int64_t pos_first = rec_pos(A, 0), pos_last = rec_pos(A, A.n_rec);   // bytes outside are in no record
 
     if (tid < 256) sm.lut[tid] = A.lut[tid];
+    // launched with programmatic stream serialisation: everything above overlaps the tail of the pre-pass kernel, whose
+    // outputs (first_rec, out_offsets) are read only behind this point (a no-op in an ordinary launch)
+    asm volatile("griddepcontrol.wait;" ::: "memory");
     if (tid == 0) sm.done_cnt = 0;
     __syncthreads();
 
