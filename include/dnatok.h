@@ -249,6 +249,21 @@ int64_t dnatok_launch_count(const dnatok_t *h);
 int dnatok_set_super_tile(dnatok_t *h, int32_t sub_tiles);
 
 /*
+ * Test / tuning knob of the strip path: 1 (default) = inputs of 4 MiB or more go to the closed-form
+ * encoder first, which assumes records laid out as an optional '>' header line followed by lines of one fixed width and
+ * checks that layout on every byte; the chained-scan encoder runs behind it only if the check failed somewhere.  2 = the
+ * same for inputs of any size (tests), 0 = the chained-scan encoder only.  Results never depend on it.  EINVAL outside 0..2.
+ */
+int dnatok_set_fast_path(dnatok_t *h, int32_t enable);
+
+/*
+ * Synchronises `stream`, then says how the last dnatok_encode call on the handle was served: 1 = by the closed-form
+ * encoder alone (the layout check held on every byte), 0 = by the chained-scan encoder (check failed, fast path off or
+ * input under the size threshold, or another mode).  Negative = DNATOK_E*.  Tests use it to tell the two apart.
+ */
+int dnatok_fast_path_taken(dnatok_t *h, void *stream);
+
+/*
  * Tuning / test knob: cap on the number of persistent CTAs the encode, BPE and pad kernels launch (0 = the
  * default, one grid's worth of resident CTAs).  Tests set 1, 2, 7 so that one CTA walks many super-tiles /
  * reads and every buffer-reuse path of the persistent kernels runs deterministically on small inputs.

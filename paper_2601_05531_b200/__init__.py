@@ -25,7 +25,7 @@ __all__ = [
     "DNATok", "Config", "Batch", "DNATokError", "lib", "library_path",
     "SINGLE_NT", "KMER", "BPE", "I16", "I32", "TAIL_PER_BASE", "TAIL_DROP", "TAIL_UNK", "PAD_LEFT", "PAD_RIGHT",
     "dnatok_create", "dnatok_destroy", "dnatok_encode", "dnatok_pad", "dnatok_stream_encode", "dnatok_check",
-    "dnatok_last_error", "dnatok_launch_count", "dnatok_version", "dnatok_config_default", "dnatok_set_super_tile", "dnatok_set_grid_cap",
+    "dnatok_last_error", "dnatok_launch_count", "dnatok_version", "dnatok_config_default", "dnatok_set_super_tile", "dnatok_set_grid_cap", "dnatok_set_fast_path", "dnatok_fast_path_taken",
     "dnatok_stream_encode_from", "dnatok_revcomp", "dnatok_decode", "dnatok_microbatch_rows", "dnatok_embed", "dnatok_widen_ids",
 ]
 
@@ -69,6 +69,7 @@ _FILL_FN = ctypes.CFUNCTYPE(ctypes.c_int, ctypes.c_void_p, ctypes.c_int64, ctype
 _MICROBATCH_FN = ctypes.CFUNCTYPE(None, ctypes.c_void_p, ctypes.c_int64, ctypes.c_int64, ctypes.c_void_p, ctypes.c_void_p)
 _lib = None
 SUPER_TILE = 0      # sub-tiles per super-tile applied to new DNATok handles (0 = automatic); a tuning knob, see dnatok.h
+FAST_PATH = 1       # dnatok_set_fast_path value applied to new DNATok handles (1 = library default; a test knob, see dnatok.h)
 GRID_CAP = 0        # cap on persistent CTAs per launch applied to new DNATok handles (0 = none); a test knob, see dnatok.h
 
 
@@ -113,6 +114,10 @@ def lib() -> ctypes.CDLL:
         L.dnatok_set_super_tile.argtypes = [vp, i32]
         L.dnatok_set_grid_cap.restype = ctypes.c_int
         L.dnatok_set_grid_cap.argtypes = [vp, i32]
+        L.dnatok_set_fast_path.restype = ctypes.c_int
+        L.dnatok_set_fast_path.argtypes = [vp, i32]
+        L.dnatok_fast_path_taken.restype = ctypes.c_int
+        L.dnatok_fast_path_taken.argtypes = [vp, vp]
         L.dnatok_launch_count.restype = i64
         L.dnatok_launch_count.argtypes = [vp]
         L.dnatok_revcomp.restype = ctypes.c_int
@@ -194,6 +199,17 @@ def dnatok_set_super_tile(h: int, sub_tiles: int) -> None:
 
 def dnatok_set_grid_cap(h: int, max_ctas: int) -> None:
     _chk(h, lib().dnatok_set_grid_cap(h, int(max_ctas)))
+
+
+def dnatok_set_fast_path(h: int, enable: int) -> None:
+    _chk(h, lib().dnatok_set_fast_path(h, int(enable)))
+
+
+def dnatok_fast_path_taken(h: int, stream: int = 0) -> bool:
+    rc = lib().dnatok_fast_path_taken(h, stream)
+    if rc < 0:
+        _chk(h, rc)
+    return rc == 1
 
 
 def dnatok_launch_count(h: int) -> int:
@@ -323,6 +339,8 @@ class DNATok:
             dnatok_set_super_tile(self.h, SUPER_TILE)
         if GRID_CAP:
             dnatok_set_grid_cap(self.h, GRID_CAP)
+        if FAST_PATH != 1:
+            dnatok_set_fast_path(self.h, FAST_PATH)
         self.id_torch_dtype = torch.int16 if self.cfg.id_dtype == I16 else torch.int32
 
     def close(self) -> None:
@@ -467,6 +485,10 @@ class DNATok:
     def check(self, stream=None) -> None:
         """Synchronise the stream and raise DNATokError if the device status word reports a failure."""
         dnatok_check(self.h, self._stream(stream))
+
+    def fast_path_taken(self, stream=None) -> bool:
+        """Synchronise the stream; True if the last encode() was served by the regular-layout encoder alone."""
+        return dnatok_fast_path_taken(self.h, self._stream(stream))
 
     @property
     def launch_count(self) -> int:

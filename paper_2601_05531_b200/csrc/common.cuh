@@ -88,6 +88,7 @@ struct EncArgs {
     unsigned long long ticket_base;
     uint32_t *status;             // device-mapped host status word
     unsigned long long *prof;     // phase timers (debug builds with -DDTK_PROF only)
+    const uint32_t *run_if;       // non-null: the chained-scan encoder runs only if *run_if != 0 (set by the regular-layout fast path)
     uint32_t gen;
     int32_t n_tiles;              // super-tiles
     int32_t S;                    // sub-tiles per super-tile (1..S_MAX)

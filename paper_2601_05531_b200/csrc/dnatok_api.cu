@@ -17,6 +17,7 @@
 #include "common.cuh"
 #include "encode_v5.cuh"
 #include "encode_v7.cuh"
+#include "encode_fasta.cuh"
 #include "ext_kernels.cuh"
 #include "pad_kernel.cuh"
 
@@ -39,6 +40,11 @@ struct EncCtx {
     uint32_t *d_status = nullptr;      // device alias of h_status
     uint32_t gen = 0;
     unsigned long long *prof = nullptr;   // phase timers of debug builds (-DDTK_PROF)
+    // regular-layout fast path (encode_fasta.cuh)
+    int32_t *fa_par = nullptr, *fa_tok = nullptr; int64_t fa_rec_cap = 0;
+    int32_t *fa_first = nullptr; int64_t fa_tile_cap = 0;
+    uint32_t *fa_flag = nullptr;
+    bool fa_tried = false;             // the last strip-path call on this context went through the regular-layout encoder
     // BPE pass scratch
     uint8_t *cls = nullptr;  int64_t cls_cap = 0;
     uint16_t *tmp_tok = nullptr;
@@ -89,6 +95,9 @@ struct dnatok {
     int enc_ctas_per_sm = 1, dense_ctas_per_sm = 1, bpe_ctas_per_sm = 1;
     bool dense = false;                // no SKIP class and strip_headers == 0: kept bases = bytes, the no-scan encoder runs
     int force_S = 0;                   // dnatok_set_super_tile: fixed super-tile size in sub-tiles (0 = automatic)
+    int fast_path = 1;                 // dnatok_set_fast_path: 1 = try the regular-layout encoder first on inputs of 4 MiB or more,
+                                       //   2 = on every input, 0 = chained-scan encoder only
+    int fasta_ctas_per_sm = 4;
     int grid_cap = 0;                  // dnatok_set_grid_cap: at most this many persistent CTAs per launch (0 = no cap)
     int64_t launches = 0;
     std::string err;
@@ -150,6 +159,7 @@ int ctx_init(dnatok_t *h, EncCtx &c) {
 void ctx_free(EncCtx &c) {
     cudaFree(c.descs); cudaFree(c.gdescs); cudaFree(c.ls); cudaFree(c.first_rec); cudaFree(c.rec_k); cudaFree(c.ticket); cudaFreeHost(c.h_status);
     cudaFree(c.prof);
+    cudaFree(c.fa_par); cudaFree(c.fa_tok); cudaFree(c.fa_first); cudaFree(c.fa_flag);
     cudaFree(c.cls); cudaFree(c.tmp_tok); cudaFree(c.koff); cudaFree(c.tok_cnt); cudaFree(c.segs); cudaFree(c.bpe_ctl); cudaFree(c.bpe_hist);
     c = EncCtx();
 }
@@ -178,6 +188,27 @@ int ctx_reserve_tiles(dnatok_t *h, EncCtx &c, int64_t n_tiles, int64_t n_rec, cu
     CU(cudaMemsetAsync(c.descs, 0, (size_t)cap * sizeof(TileDesc), st));
     CU(cudaMemsetAsync(c.ls, 0, (size_t)cap * sizeof(uint32_t), st));
     c.descs_cap = cap;
+    return DNATOK_OK;
+}
+
+int ctx_reserve_fasta(dnatok_t *h, EncCtx &c, int64_t n_rec, int64_t n_wtiles, cudaStream_t st) {
+    if (!c.fa_flag) CU(cudaMallocAsync((void **)&c.fa_flag, 16, st));
+    if (n_rec + 1 > c.fa_rec_cap) {
+        if (c.fa_par) CU(cudaFreeAsync(c.fa_par, st));
+        if (c.fa_tok) CU(cudaFreeAsync(c.fa_tok, st));
+        c.fa_par = nullptr; c.fa_tok = nullptr; c.fa_rec_cap = 0;
+        const int64_t cap = n_rec + n_rec / 4 + 1024;
+        CU(cudaMallocAsync((void **)&c.fa_par, (size_t)cap * 4 * sizeof(int32_t), st));
+        CU(cudaMallocAsync((void **)&c.fa_tok, (size_t)cap * sizeof(int32_t), st));
+        c.fa_rec_cap = cap;
+    }
+    if (n_wtiles + 1 > c.fa_tile_cap) {
+        if (c.fa_first) CU(cudaFreeAsync(c.fa_first, st));
+        c.fa_first = nullptr; c.fa_tile_cap = 0;
+        const int64_t cap = n_wtiles + n_wtiles / 4 + 1024;
+        CU(cudaMallocAsync((void **)&c.fa_first, (size_t)cap * sizeof(int32_t), st));
+        c.fa_tile_cap = cap;
+    }
     return DNATOK_OK;
 }
 
@@ -220,20 +251,47 @@ void launch_dense(const EncArgs &a, int kk, int grid, cudaStream_t st) {
         default: launch_pdl(v7::encode_tiles_v7<IdT, wide ? -1 : 0, true>, grid, v7::NT7, sizeof(v7::Smem7), st, a, true); break;
     }
 }
+template <typename K, typename... Args>
+void launch_pdl1(K kernel, int grid, int block, size_t smem, cudaStream_t st, bool pdl, Args... args) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)grid); cfg.blockDim = dim3((unsigned)block); cfg.dynamicSmemBytes = smem; cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr; cfg.numAttrs = pdl ? 1 : 0;
+    cudaLaunchKernelEx(&cfg, kernel, args...);
+}
 template <typename IdT>
-void launch_strip(const EncArgs &a, int kk, int grid, cudaStream_t st) {
+void launch_fasta(const fa::FastaArgs &f, int kk, int grid, cudaStream_t st) {
+    using namespace dtk::fa;
+    constexpr bool wide = sizeof(IdT) >= 2;
+    const size_t sm = sizeof(SmemFa);
+    switch (wide ? kk : 0) {
+        case 0: launch_pdl1(encode_fasta_kernel<IdT, 0>, grid, FW_WARPS * 32, sm, st, true, f); break;
+        case 1: launch_pdl1(encode_fasta_kernel<IdT, wide ? 1 : 0>, grid, FW_WARPS * 32, sm, st, true, f); break;
+        case 2: launch_pdl1(encode_fasta_kernel<IdT, wide ? 2 : 0>, grid, FW_WARPS * 32, sm, st, true, f); break;
+        case 3: launch_pdl1(encode_fasta_kernel<IdT, wide ? 3 : 0>, grid, FW_WARPS * 32, sm, st, true, f); break;
+        case 4: launch_pdl1(encode_fasta_kernel<IdT, wide ? 4 : 0>, grid, FW_WARPS * 32, sm, st, true, f); break;
+        case 5: launch_pdl1(encode_fasta_kernel<IdT, wide ? 5 : 0>, grid, FW_WARPS * 32, sm, st, true, f); break;
+        case 6: launch_pdl1(encode_fasta_kernel<IdT, wide ? 6 : 0>, grid, FW_WARPS * 32, sm, st, true, f); break;
+        case 8: launch_pdl1(encode_fasta_kernel<IdT, wide ? 8 : 0>, grid, FW_WARPS * 32, sm, st, true, f); break;
+        default: launch_pdl1(encode_fasta_kernel<IdT, wide ? -1 : 0>, grid, FW_WARPS * 32, sm, st, true, f); break;
+    }
+}
+template <typename IdT>
+void launch_strip(const EncArgs &a, int kk, int grid, cudaStream_t st, bool chained) {
     using namespace dtk::v5;
     constexpr bool wide = sizeof(IdT) >= 2;
     switch (wide ? kk : 0) {
-        case 0: launch_pdl(encode_tiles_v5<IdT, 0>, grid, NT, sizeof(Smem5), st, a, a.first_rec != nullptr); break;
-        case 1: launch_pdl(encode_tiles_v5<IdT, wide ? 1 : 0>, grid, NT, sizeof(Smem5), st, a, a.first_rec != nullptr); break;
-        case 2: launch_pdl(encode_tiles_v5<IdT, wide ? 2 : 0>, grid, NT, sizeof(Smem5), st, a, a.first_rec != nullptr); break;
-        case 3: launch_pdl(encode_tiles_v5<IdT, wide ? 3 : 0>, grid, NT, sizeof(Smem5), st, a, a.first_rec != nullptr); break;
-        case 4: launch_pdl(encode_tiles_v5<IdT, wide ? 4 : 0>, grid, NT, sizeof(Smem5), st, a, a.first_rec != nullptr); break;
-        case 5: launch_pdl(encode_tiles_v5<IdT, wide ? 5 : 0>, grid, NT, sizeof(Smem5), st, a, a.first_rec != nullptr); break;
-        case 6: launch_pdl(encode_tiles_v5<IdT, wide ? 6 : 0>, grid, NT, sizeof(Smem5), st, a, a.first_rec != nullptr); break;
-        case 8: launch_pdl(encode_tiles_v5<IdT, wide ? 8 : 0>, grid, NT, sizeof(Smem5), st, a, a.first_rec != nullptr); break;
-        default: launch_pdl(encode_tiles_v5<IdT, wide ? -1 : 0>, grid, NT, sizeof(Smem5), st, a, a.first_rec != nullptr); break;
+        case 0: launch_pdl(encode_tiles_v5<IdT, 0>, grid, NT, sizeof(Smem5), st, a, a.first_rec != nullptr || chained); break;
+        case 1: launch_pdl(encode_tiles_v5<IdT, wide ? 1 : 0>, grid, NT, sizeof(Smem5), st, a, a.first_rec != nullptr || chained); break;
+        case 2: launch_pdl(encode_tiles_v5<IdT, wide ? 2 : 0>, grid, NT, sizeof(Smem5), st, a, a.first_rec != nullptr || chained); break;
+        case 3: launch_pdl(encode_tiles_v5<IdT, wide ? 3 : 0>, grid, NT, sizeof(Smem5), st, a, a.first_rec != nullptr || chained); break;
+        case 4: launch_pdl(encode_tiles_v5<IdT, wide ? 4 : 0>, grid, NT, sizeof(Smem5), st, a, a.first_rec != nullptr || chained); break;
+        case 5: launch_pdl(encode_tiles_v5<IdT, wide ? 5 : 0>, grid, NT, sizeof(Smem5), st, a, a.first_rec != nullptr || chained); break;
+        case 6: launch_pdl(encode_tiles_v5<IdT, wide ? 6 : 0>, grid, NT, sizeof(Smem5), st, a, a.first_rec != nullptr || chained); break;
+        case 8: launch_pdl(encode_tiles_v5<IdT, wide ? 8 : 0>, grid, NT, sizeof(Smem5), st, a, a.first_rec != nullptr || chained); break;
+        default: launch_pdl(encode_tiles_v5<IdT, wide ? -1 : 0>, grid, NT, sizeof(Smem5), st, a, a.first_rec != nullptr || chained); break;
     }
 }
 
@@ -265,6 +323,7 @@ int launch_tiles(dnatok_t *h, EncCtx &c, const EncParams &prm, const uint8_t *d_
     a.ids = ids; a.ids_cap = ids_cap; a.out_off = out_off; a.out_bias = 0;
     a.lut = h->d_lut; a.descs = c.descs; a.gdescs = c.gdescs; a.ls = c.ls; a.rec_k = c.rec_k; a.first_rec = c.first_rec; a.ticket = c.ticket; a.ticket_base = c.ticket_base;
     a.status = c.d_status; a.prof = c.prof; a.gen = c.gen; a.n_tiles = (int32_t)n_tiles; a.prm = prm;
+    a.run_if = nullptr;
     int grid = (int)std::min<int64_t>(n_tiles, slots);
     if (h->grid_cap > 0) grid = std::min(grid, h->grid_cap);
     // table-driven ids are compiled into the run-time-switch variant only (the per-k variants stay lean)
@@ -277,15 +336,43 @@ int launch_tiles(dnatok_t *h, EncCtx &c, const EncParams &prm, const uint8_t *d_
         h->launches += 1;
         launch_dense<IdT>(a, kk, grid, st);
     } else {
+        bool chained = false;                                 // the kernels below follow kernels of this call
+        c.fa_tried = false;
+        if ((h->fast_path == 2 || (h->fast_path == 1 && n_bytes >= (4ll << 20))) && n_rec < (1ll << 31)) {
+            // regular-layout fast path first (encode_fasta.cuh); the chained-scan encoder behind it runs only if the layout
+            // check failed somewhere
+            const int64_t n_wtiles = (a.p_end + fa::FW_TILE - 1) / fa::FW_TILE;
+            const int64_t nb_scan = std::max<int64_t>(1, (n_rec + fa::OS_BLK - 1) / fa::OS_BLK);
+            rc = ctx_reserve_tiles(h, c, std::max(n_tiles, nb_scan), n_rec, st); if (rc) return rc;
+            rc = ctx_reserve_fasta(h, c, n_rec, n_wtiles, st); if (rc) return rc;
+            a.descs = c.descs; a.gdescs = c.gdescs; a.ls = c.ls; a.rec_k = c.rec_k; a.first_rec = c.first_rec;
+            CU(cudaMemsetAsync(c.fa_flag, 0, 16, st));
+            fa::FastaArgs f;
+            f.e = a; f.par = c.fa_par; f.rec_tok = c.fa_tok; f.wt_first = c.fa_first; f.irregular = c.fa_flag;
+            f.n_wtiles = (int32_t)n_wtiles;
+            const int64_t nthr = std::max<int64_t>(n_rec, n_wtiles);
+            fa::fasta_parse_kernel<<<(unsigned)std::max<int64_t>(1, (nthr + 255) / 256), 256, 0, st>>>(f);
+            launch_pdl1(fa::offsets_scan_kernel, (int)nb_scan, fa::OS_NT, 0, st, true, (const int32_t *)c.fa_tok, n_rec, out_off, (int64_t)0, c.descs, a.gen, c.d_status);
+            int fgrid = (int)std::min<int64_t>((n_wtiles + fa::FW_WARPS - 1) / fa::FW_WARPS, (int64_t)h->sm_count * h->fasta_ctas_per_sm);
+            fgrid = std::max(fgrid, 1);
+            if (h->grid_cap > 0) fgrid = std::min(fgrid, h->grid_cap);
+            launch_fasta<IdT>(f, kk, fgrid, st);
+            CU(cudaGetLastError());
+            h->launches += 3;
+            rc = ctx_next_gen(h, c, st); if (rc) return rc;      // the scan above used this generation's chain words
+            a.gen = c.gen; a.run_if = c.fa_flag;
+            chained = true;
+            c.fa_tried = true;
+        }
         // an input that gives every CTA at most one tile is encoded in ONE launch: the record range of a tile is searched
         // inside the kernel instead of by the pre-pass (SURVEY.md section 7 hard part 6)
         if (n_tiles <= slots && n_rec <= (1 << 16)) a.first_rec = nullptr;
         else {
-            v5::tile_first_rec_kernel<<<nb_first, 256, 0, st>>>(a);
+            launch_pdl1(v5::tile_first_rec_kernel, (int)nb_first, 256, 0, st, chained, a);
             CU(cudaGetLastError());
             h->launches += 1;
         }
-        launch_strip<IdT>(a, kk, grid, st);
+        launch_strip<IdT>(a, kk, grid, st, chained);
     }
     CU(cudaGetLastError());
     c.ticket_base += (unsigned long long)n_tiles + (unsigned long long)grid;
@@ -665,7 +752,17 @@ int dnatok_create(const dnatok_config *cfg_in, int device, dnatok_t **out) {
         for (const void *kf : k7)
             if (cudaFuncSetAttribute(kf, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(v7::Smem7)) != cudaSuccess)
                 return bail(DNATOK_ECUDA);
+#define DTK_FA(T) (const void *)fa::encode_fasta_kernel<T, 0>, (const void *)fa::encode_fasta_kernel<T, 1>, (const void *)fa::encode_fasta_kernel<T, 2>, \
+                  (const void *)fa::encode_fasta_kernel<T, 3>, (const void *)fa::encode_fasta_kernel<T, 4>, (const void *)fa::encode_fasta_kernel<T, 5>, \
+                  (const void *)fa::encode_fasta_kernel<T, 6>, (const void *)fa::encode_fasta_kernel<T, 8>, (const void *)fa::encode_fasta_kernel<T, -1>
+        const void *kfa[] = {DTK_FA(int32_t), DTK_FA(int16_t), (const void *)fa::encode_fasta_kernel<uint8_t, 0>};
+#undef DTK_FA
+        for (const void *kf : kfa)
+            if (cudaFuncSetAttribute(kf, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(fa::SmemFa)) != cudaSuccess)
+                return bail(DNATOK_ECUDA);
         int nb = 0;
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, fa::encode_fasta_kernel<int32_t, -1>, fa::FW_WARPS * 32, sizeof(fa::SmemFa));
+        h->fasta_ctas_per_sm = std::max(nb, 1);
         cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, v5::encode_tiles_v5<int32_t, -1>, NT, sizeof(v5::Smem5));
         h->enc_ctas_per_sm = std::max(nb, 1);
         cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, v7::encode_tiles_v7<int32_t, -1, true>, v7::NT7, sizeof(v7::Smem7));
@@ -862,6 +959,23 @@ int dnatok_set_super_tile(dnatok_t *h, int32_t sub_tiles) {
     if (sub_tiles < 0 || sub_tiles > S_MAX) return fail(h, DNATOK_EINVAL, "dnatok_set_super_tile: sub_tiles must be in 0..%d", S_MAX);
     h->force_S = sub_tiles;
     return DNATOK_OK;
+}
+
+int dnatok_set_fast_path(dnatok_t *h, int32_t enable) {
+    if (!h) return DNATOK_EINVAL;
+    if (enable < 0 || enable > 2) return fail(h, DNATOK_EINVAL, "dnatok_set_fast_path: 0, 1 or 2");
+    h->fast_path = enable;
+    return DNATOK_OK;
+}
+
+int dnatok_fast_path_taken(dnatok_t *h, void *stream) {
+    if (!h) return DNATOK_EINVAL;
+    USE_DEVICE(h);
+    CU(cudaStreamSynchronize((cudaStream_t)stream));
+    if (!h->ctx.fa_tried) return 0;
+    uint32_t flag = 0;
+    CU(cudaMemcpy(&flag, h->ctx.fa_flag, sizeof(flag), cudaMemcpyDeviceToHost));
+    return flag == 0u ? 1 : 0;
 }
 
 int dnatok_set_grid_cap(dnatok_t *h, int32_t max_ctas) {

@@ -469,6 +469,8 @@ __device__ __forceinline__ void emit_segments(const EncArgs &A, const uint32_t *
 // first_rec[t] = first r in [0, n_rec] with position >= t * S * TB (n_rec + 1 if none); first_rec[n_tiles] = n_rec + 1
 __global__ void __launch_bounds__(256) tile_first_rec_kernel(const __grid_constant__ EncArgs A) {
     asm volatile("griddepcontrol.launch_dependents;" ::: "memory");   // the encode kernel may start its prologue now
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+    if (A.run_if && *A.run_if == 0u) return;                           // the regular-layout fast path has done the work
     const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (t > A.n_tiles) return;
     int64_t lo = 0, hi = A.n_rec + 1;
@@ -682,6 +684,11 @@ __global__ void __launch_bounds__(NT, 1024 / NT) encode_tiles_v5(const __grid_co
     // launched with programmatic stream serialisation: everything above overlaps the tail of the pre-pass kernel, whose
     // outputs (first_rec, out_offsets) are read only behind this point (a no-op in an ordinary launch)
     asm volatile("griddepcontrol.wait;" ::: "memory");
+    if (A.run_if && *A.run_if == 0u) {
+        // the regular-layout fast path (encode_fasta.cuh) has encoded this input: only the ticket counter is kept in step
+        if (blockIdx.x == 0 && tid == 0) atomicAdd(A.ticket, (unsigned long long)A.n_tiles + gridDim.x);
+        return;
+    }
     __syncthreads();
     unsigned long long next_ticket = 0;
     if (warp == NW - 1) {

@@ -17,11 +17,13 @@ def golden_dir():
     return os.path.join(ROOT, "tests", "golden")
 
 
-@pytest.fixture(params=[0, 1, 2, 4], ids=lambda s: f"S{s}")
+@pytest.fixture(params=[0, 1, 2, 4, "chained"], ids=lambda s: f"S{s}")
 def super_tile(request):
-    """GPU parity must hold for every super-tile size of the single-pass encoder (0 = automatic)."""
+    """GPU parity must hold for every super-tile size of the single-pass encoder (0 = automatic), with the regular-layout
+    fast path in front of it (the default) and, in the "chained" variant, with the chained-scan encoder alone."""
     import paper_2601_05531_b200 as dn
-    old = dn.SUPER_TILE
-    dn.SUPER_TILE = request.param
+    old, oldf = dn.SUPER_TILE, dn.FAST_PATH
+    dn.SUPER_TILE = 0 if request.param == "chained" else request.param
+    dn.FAST_PATH = 0 if request.param == "chained" else 2           # 2: the fast path on inputs of any size
     yield request.param
-    dn.SUPER_TILE = old
+    dn.SUPER_TILE, dn.FAST_PATH = old, oldf
