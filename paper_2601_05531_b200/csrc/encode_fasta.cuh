@@ -8,14 +8,14 @@
 //   fasta_parse_kernel    one thread per record reads its header line and its first sequence line (bounded), stores (B, W) and
 //                         the record's token count; one thread per warp tile finds the record that holds the tile's first byte
 //   offsets_scan_kernel   token counts -> out_offsets (chained scan over blocks of 2048 records)
-//   encode_fasta_kernel   every WARP encodes whole 8 KiB tiles on its own: per record piece inside the tile it classifies 64
+//   encode_fasta_kernel   every WARP encodes whole 16 KiB tiles on its own: per record piece inside the tile it classifies 64
 //                         bytes per lane exactly as encode_v5.cuh does, takes the keep mask from the closed form, compacts in
 //                         registers, appends at the closed-form position into the warp's private kept-base stream in shared
 //                         memory (interior words by shuffle + plain store, the two edge words by atomicOr), reads 64 bytes past
 //                         the piece for the windows that straddle its end, and cuts the tokens whose first base lies in the piece.
 // The closed form is an ASSUMPTION about the bytes, and every lane checks it on the bytes it holds: the SKIP bytes of the body
 // must be exactly the predicted newlines, and no body line may start with '>' (which would be a second header line).  Any
-// violation, a header or first line longer than the parse bound, or more than 8 records in one tile, sets *irregular; the
+// violation, a header or first line longer than the parse bound, or more than 16 records in one tile, sets *irregular; the
 // chained-scan encoder of encode_v5.cuh is launched behind this kernel in every call and returns at once unless the flag
 // is set, in which case it encodes the whole input again (the result is then its result).  The LUT stays the specification:
 // a table with other SKIP bytes, or one that does not skip '\n', simply fails the check wherever such bytes occur.
@@ -28,15 +28,15 @@ namespace fa {
 
 using namespace dtk::v5;
 
-constexpr int FW_CHUNKS = 4;                        // 2 KiB chunks per warp tile
-constexpr int FW_TILE = FW_CHUNKS * WB;             // bytes per warp tile (8 KiB)
+constexpr int FW_CHUNKS = 8;                        // 2 KiB chunks per warp tile
+constexpr int FW_TILE = FW_CHUNKS * WB;             // bytes per warp tile (16 KiB)
 constexpr int FW_HALO = 64;                         // bytes read past a piece that ends at the tile's end
 constexpr int FW_BASES = FW_TILE + FW_HALO;
 constexpr int FW_CW = FW_BASES / 16 + 8;            // code words of a warp's stream (+ over-read slack)
 constexpr int FW_FW = FW_BASES / 32 + 10;
 constexpr int FW_WORDS = FW_CW + FW_FW;
 constexpr int FW_WARPS = 8;                         // warps per CTA
-constexpr int FW_MAXSEG = 8;                        // records per warp tile the fast path accepts
+constexpr int FW_MAXSEG = 2 * FW_CHUNKS;            // records per warp tile the fast path accepts
 constexpr int FW_HDR_BOUND = 4096;                  // bytes the parse reads looking for the end of a header line
 constexpr int FW_LINE_BOUND = 512;                  //   ... and for the end of the first sequence line
 static_assert(FW_WORDS % 4 == 0, "per-warp streams stay 16-byte aligned");
@@ -315,7 +315,8 @@ __global__ void __launch_bounds__(FW_WARPS * 32, 3) encode_fasta_kernel(const __
             const int B = __ldg(F.par + 4 * r), W = __ldg(F.par + 4 * r + 1), Z = __ldg(F.par + 4 * r + 2);
             const uint32_t d = (uint32_t)W + 1u;
             const float dinv = 1.0f / (float)d;
-            // c / d for c < d + 2112 in one multiply: exact while c * (dmul * d - 2^32) < 2^32, i.e. for every d up to 2^16
+            // c / d in one multiply for the columns c < d + FW_TILE + FW_HALO met below: exact while c * (dmul * d - 2^32) < 2^32
+            // (every d up to 2^14) or c < 2 d - 1 (the larger d)
             const uint32_t dmul = d <= 65536u ? (uint32_t)(0x100000000ull / d) + 1u : 0u;
             const int64_t bend = re - Z;                                         // end of the body (the record's final line end set apart)
             const int64_t sbb = sb < bend ? sb : bend;
@@ -353,17 +354,22 @@ __global__ void __launch_bounds__(FW_WARPS * 32, 3) encode_fasta_kernel(const __
                 // ---- interior chunk of wrapped lines (the bulk of a FASTA record): all 2 KiB are body bytes of the piece, lines
                 // are longer than a lane, so each lane holds 64 body bytes and at most one predicted line end.  Streamlined:
                 // no per-byte flags, no masks; falls through to the general code below if any lane fails the layout check ----
-                if (d >= 65u && P.fast_lut && nl_skips && c_rel >= sa_rel && c_rel + WB <= he_rel && c_rel + WB <= end_rel && yb + c_rel >= 0) {
+                // The 64 bytes read past the tile's end take the same road with one active lane (nact = active lanes).
+                const int left = he_rel - c_rel;
+                if (d >= 65u && P.fast_lut && nl_skips && c_rel >= sa_rel && (left >= WB || (left & 63) == 0) &&
+                    c_rel + min(left, WB) <= end_rel && yb + c_rel >= 0) {
+                    const int nact = left >= WB ? 32 : left >> 6;
+                    const bool on = lane < nact;
                     uint4 v[4];
                     {
                         const uint4 *src = reinterpret_cast<const uint4 *>(tb + q_rel);
 #pragma unroll
-                        for (int j = 0; j < 4; ++j) v[j] = __ldg(src + j);
+                        for (int j = 0; j < 4; ++j) v[j] = on ? __ldg(src + j) : make_uint4(0x41414141u, 0x41414141u, 0x41414141u, 0x41414141u);
                     }
                     const uint32_t c = col_p + ((uint32_t)(yb + q_rel) - y_p);   // column counted from the piece's first line
                     const uint32_t q = dmul ? __umulhi(c, dmul) : (uint32_t)(c >= d);
                     const uint32_t col = c - q * d;
-                    const uint32_t tn = (uint32_t)W - col;                       // lane index of the predicted line end (>= 64: none)
+                    const uint32_t tn = on ? (uint32_t)W - col : 64u;            // lane index of the predicted line end (>= 64: none)
                     const int u = (int)(q * (uint32_t)W + col) - (int)col_p;
                     uint32_t C[4], dd[16];
                     {
@@ -421,11 +427,13 @@ __global__ void __launch_bounds__(FW_WARPS * 32, 3) encode_fasta_kernel(const __
                         uint32_t part = li == 2 ? w2 : (li == 3 ? w3 : w4);
                         if ((cend & 31) == 0) part = 0u;
                         const uint32_t prev = __shfl_up_sync(FULL, part, 1);
-                        if (lane == 0) { if (w0) atomicOr(&cw[cw0], w0); } else cw[cw0] = w0 | prev;
-                        cw[cw0 + 1] = w1;
-                        if (cend >= 96) cw[cw0 + 2] = w2;
-                        if (cend >= 128) cw[cw0 + 3] = w3;
-                        if (lane == 31 && part) atomicOr(&cw[cw0 + li], part);
+                        if (on) {
+                            if (lane == 0) { if (w0) atomicOr(&cw[cw0], w0); } else cw[cw0] = w0 | prev;
+                            cw[cw0 + 1] = w1;
+                            if (cend >= 96) cw[cw0 + 2] = w2;
+                            if (cend >= 128) cw[cw0 + 3] = w3;
+                            if (lane == nact - 1 && part) atomicOr(&cw[cw0 + li], part);
+                        }
                         continue;
                     }
                 }

@@ -99,7 +99,7 @@ def test_records_without_header_or_last_line_end():
 def test_body_lengths_that_are_multiples_of_the_width():
     rng = random.Random(2)
     recs = []
-    for n in (60, 120, 600, 6000, 59, 60 * 137, 61, 1, 0):                   # at most 8 records touch one 8 KiB tile
+    for n in (60, 120, 600, 6000, 59, 60 * 137, 61, 1, 0):                   # at most 16 records touch one 16 KiB tile
         seq = "".join(rng.choice("ACGT") for _ in range(n))
         recs.append((">x\n" + "".join(seq[j:j + 60] + "\n" for j in range(0, n, 60))).encode())
     run(b"".join(recs), np.cumsum([0] + [len(r) for r in recs]), True, mode="kmer", k=6)
@@ -121,7 +121,7 @@ def test_header_only_empty_and_unterminated_header_records():
     # "\nACGT\n": a body that starts with an empty line is not regular -- the call as a whole falls back
     run(b"".join(recs), offs, False, mode="kmer", k=3)
     recs.remove(b"\nACGT\n")
-    for part in (recs[:6], recs[5:]):                                          # at most 8 records per 8 KiB tile are taken
+    for part in (recs[:6], recs[5:]):                                          # at most 16 records per 16 KiB tile are taken
         offs = np.cumsum([0] + [len(r) for r in part])
         run(b"".join(part), offs, True, mode="kmer", k=3)
         run(b"".join(part), offs, True, mode="single_nt")
@@ -149,9 +149,9 @@ def test_header_lengths_up_to_the_parse_bound():
     run(long_hdr + b"".join(recs), np.cumsum([0, len(long_hdr)] + [len(r) for r in recs]), False, mode="kmer", k=6)
 
 
-def test_up_to_eight_records_per_warp_tile_are_taken_and_more_fall_back():
+def test_up_to_sixteen_records_per_warp_tile_are_taken_and_more_fall_back():
     rng = random.Random(6)
-    data, offs = fasta(rng, 64, 60, 1300, 1500)                               # ~1.4 KiB records: at most 7 pieces per 8 KiB
+    data, offs = fasta(rng, 64, 60, 1300, 1500)                               # ~1.4 KiB records: at most 13 pieces per 16 KiB tile
     run(data, offs, True, mode="kmer", k=6)
     data, offs = fasta(rng, 400, 60, 0, 300)                                  # dozens of records per tile
     run(data, offs, False, mode="kmer", k=6)
@@ -173,7 +173,7 @@ def regular_input(seed, n_rec=6, W=60):
 
 
 def edge_positions(data, offs):
-    """bytes next to warp-tile (8 KiB) and chunk (2 KiB) edges, record edges, and the ends of the input"""
+    """bytes next to warp-tile (16 KiB) and chunk (2 KiB) edges, record edges, and the ends of the input"""
     pos = set()
     for e in list(range(0, data.size, 2048)) + list(offs) + [data.size]:
         for dlt in (-66, -65, -64, -63, -17, -16, -2, -1, 0, 1, 2, 15, 16, 17, 63, 64, 65):
