@@ -280,7 +280,7 @@ __global__ void __launch_bounds__(FW_WARPS * 32, 3) encode_fasta_kernel(const __
     const EncArgs &A = F.e;
     const EncParams &P = A.prm;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int k = P.k;
+    const int k = KK > 0 ? KK : (P.mode == MODE_KMER ? P.k : 1);       // a compile-time constant in the per-k variants
     const int kk = P.mode == MODE_KMER ? k : 0;
     const bool affine = P.nt_ids[1] == P.nt_ids[0] + 1 && P.nt_ids[2] == P.nt_ids[0] + 2 && P.nt_ids[3] == P.nt_ids[0] + 3;
     const bool vec_ok = (reinterpret_cast<uintptr_t>(A.ids) & 15) == 0 &&
@@ -314,7 +314,6 @@ __global__ void __launch_bounds__(FW_WARPS * 32, 3) encode_fasta_kernel(const __
             if (++nseg > FW_MAXSEG) { irregular = true; break; }
             const int B = __ldg(F.par + 4 * r), W = __ldg(F.par + 4 * r + 1), Z = __ldg(F.par + 4 * r + 2);
             const uint32_t d = (uint32_t)W + 1u;
-            const float dinv = 1.0f / (float)d;
             // c / d in one multiply for the columns c < d + FW_TILE + FW_HALO met below: exact while c * (dmul * d - 2^32) < 2^32
             // (every d up to 2^14) or c < 2 d - 1 (the larger d)
             const uint32_t dmul = d <= 65536u ? (uint32_t)(0x100000000ull / d) + 1u : 0u;
@@ -330,17 +329,19 @@ __global__ void __launch_bounds__(FW_WARPS * 32, 3) encode_fasta_kernel(const __
             // body index, line and column of the piece's first body byte; bases of the record in front of / through the piece
             const uint32_t y_p = (uint32_t)(sa - rs > B ? sa - rs - B : 0);
             const uint32_t line_p = y_p / d, col_p = y_p - line_p * d;
-            const int64_t K0 = (int64_t)line_p * W + col_p;
+            // (a record is shorter than 2^31 bytes -- the parse kernel flags anything longer -- so base counts fit 32 bits)
+            const uint32_t K0 = line_p * (uint32_t)W + col_p;
             const uint32_t y_e = (uint32_t)(sbb - rs > B ? sbb - rs - B : 0);
             const uint32_t line_e = y_e / d, col_e = y_e - line_e * d;
-            const int nK = (int)((int64_t)line_e * W + col_e - K0);              // bases of the piece
+            const int nK = (int)(line_e * (uint32_t)W + col_e - K0);             // bases of the piece
             // windows of the record: only matters when the record ends near the piece
-            int64_t nwin = 0x7fffffffffffll, n_r = 0x7fffffffffffll;
+            constexpr uint32_t FAR = 0xffffffffu;
+            uint32_t nwin = FAR, n_r = FAR;
             if (re - sb < 2 * FW_HALO) {
                 const uint32_t y_r = (uint32_t)(bend - rs > B ? bend - rs - B : 0);
                 const uint32_t line_r = y_r / d, col_r = y_r - line_r * d;
-                n_r = (int64_t)line_r * W + col_r;
-                nwin = P.mode == MODE_KMER ? n_r / k : n_r;
+                n_r = line_r * (uint32_t)W + col_r;
+                nwin = n_r / (uint32_t)k;
             }
             const int64_t T_r = __ldcg(A.out_off + r);
             // the warp's stream starts empty (edge words are OR-ed in)
@@ -456,9 +457,8 @@ __global__ void __launch_bounds__(FW_WARPS * 32, 3) encode_fasta_kernel(const __
                     range = (i1 == 0 && ib == 64) ? ~0ull : (from_pos(i1) & ~from_pos(ib));
                     const uint32_t y1 = (uint32_t)(yb + q_rel + i1);             // body index of byte i1
                     const uint32_t c = col_p + (y1 - y_p);                       // column counted from the piece's first line
-                    uint32_t q = (uint32_t)((float)c * dinv);                    // c / d: the estimate is off by one at most
-                    int32_t col = (int32_t)(c - q * d);
-                    if (col < 0) { col += (int32_t)d; --q; } else if ((uint32_t)col >= d) { col -= (int32_t)d; ++q; }
+                    const uint32_t q = dmul ? __umulhi(c, dmul) : (uint32_t)(c >= d);
+                    const int32_t col = (int32_t)(c - q * d);
                     Kp = range;
                     const uint32_t t0 = (uint32_t)i1 + ((uint32_t)W - (uint32_t)col);
                     if (t0 < (uint32_t)ib) {
@@ -610,10 +610,10 @@ __global__ void __launch_bounds__(FW_WARPS * 32, 3) encode_fasta_kernel(const __
             __syncwarp();
             // ---- tokens whose first base lies in the piece: record base K0 + i sits at stream position i ---------------------
             // windows j of the record with K0 <= j k < K0 + nK, as piece-relative first bases u = j k - K0
-            const int ufirst = (int)((k - (int)(K0 % k)) % k);                   // stream position of the first window that starts here
-            const int64_t jfirst = (K0 + ufirst) / k;                            //   and its index in the record
-            int nwp = ufirst < nK ? (nK - ufirst + k - 1) / k : 0;               // windows that start in the piece
-            if (jfirst + nwp > nwin) nwp = nwin > jfirst ? (int)(nwin - jfirst) : 0;
+            const uint32_t jfirst = (K0 + (uint32_t)k - 1u) / (uint32_t)k;       // first window of the record that starts in the piece
+            const int ufirst = (int)(jfirst * (uint32_t)k - K0);                 //   and the stream position of its first base
+            int nwp = ufirst < nK ? (int)((uint32_t)(nK - ufirst + k - 1) / (uint32_t)k) : 0;   // windows that start in the piece
+            if (nwin != FAR && jfirst + (uint32_t)nwp > nwin) nwp = nwin > jfirst ? (int)(nwin - jfirst) : 0;
             const int64_t g0 = T_r + jfirst;                                     // global token index of the first of them
             IdT *const idp = ids + g0;
             int xa = nwp, xb = nwp;                                              // windows [xa, xb) go through the 16-byte group cutter
@@ -633,11 +633,11 @@ __global__ void __launch_bounds__(FW_WARPS * 32, 3) encode_fasta_kernel(const __
                     store_id<IdT>(A, g0 + x, w_window_id(P, cw, fw, ufirst + x * k));
                 }
             }
-            if (P.mode == MODE_KMER && n_r < 0x7fffffffffffll) {
+            if (P.mode == MODE_KMER && n_r != FAR) {
                 // the n mod k trailing bases of the record, if they lie in the piece
-                const int64_t tb0 = nwin * k;
+                const int64_t tb0 = (int64_t)nwin * k;
                 if (P.tail_policy == TAIL_PER_BASE) {
-                    const int64_t b0 = K0 > tb0 ? K0 : tb0, b1 = K0 + nK < n_r ? K0 + nK : n_r;
+                    const int64_t b0 = K0 > tb0 ? K0 : tb0, b1 = (int64_t)K0 + nK < n_r ? (int64_t)K0 + nK : n_r;
                     for (int64_t bb = b0 + lane; bb < b1; bb += 32) {
                         const uint32_t c = w_class(cw, fw, (int)(bb - K0));
                         const int32_t id = c <= CLS_N ? (P.remap4 ? P.nt_ids[c] : (int32_t)(P.base_id + P.four_k + c)) : P.unk_id;
