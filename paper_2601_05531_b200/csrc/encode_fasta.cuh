@@ -53,8 +53,22 @@ struct FastaArgs {
 
 struct SmemFa {
     uint32_t strm[FW_WARPS][FW_WORDS];
+    uint4 stage[FW_WARPS][4 * 32];      // the chunk a warp works on next, copied asynchronously: 16-byte unit j of lane l at [j * 32 + l]
     uint8_t lut[256];
 };
+
+// this lane's 64 bytes of the chunk at tile offset c (tile base tb) -> the warp's staging buffer; bytes from tile offset lim on
+// read as zero.  One cp.async group per chunk.
+__device__ __forceinline__ void stage_chunk(uint4 *stg, const uint8_t *tb, int c, int lim, int lane) {
+    const int q = c + lane * LB;
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+        const uint32_t dst = (uint32_t)__cvta_generic_to_shared(stg + j * 32 + lane);
+        const int sz = q + 16 * j < lim ? 16 : 0;
+        asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(dst), "l"(tb + q + 16 * j), "r"(sz) : "memory");
+    }
+    asm volatile("cp.async.commit_group;" ::: "memory");
+}
 
 // bases among the first y body bytes of a record with line width W
 __device__ __forceinline__ int64_t kept_before(int64_t y, int W) {
@@ -293,17 +307,37 @@ __global__ void __launch_bounds__(FW_WARPS * 32, 3) encode_fasta_kernel(const __
     IdT *const ids = reinterpret_cast<IdT *>(A.ids);
     bool irregular = false;
     const bool nl_skips = sm.lut[(uint8_t)'\n'] == CLS_SKIP;
+    // x >> 1 and x >> 2 as multiply-high by 2^31 and 2^30: the shifts of the classification leave the ALU pipe, which bounds
+    // this kernel, for the FMA pipe, which idles (IMAD.HI issues at half rate, measured, and overlaps LOP3 fully).  The factors
+    // are kept opaque so that the compiler does not turn the multiplies back into shifts.
+    const uint32_t mh31 = 0x80000000u | (uint32_t)(F.n_wtiles < 0), mh30 = mh31 >> 1;
 
     const int64_t n_warps = (int64_t)gridDim.x * FW_WARPS;
 #pragma unroll 1
     for (int64_t tile = (int64_t)blockIdx.x * FW_WARPS + warp; tile < F.n_wtiles; tile += n_warps) {
         const int64_t ts = tile * FW_TILE, te = ts + FW_TILE < A.p_end ? ts + FW_TILE : A.p_end;
         int nseg = 0;
+#ifndef FW_PREFETCH
+#define FW_PREFETCH 2
+#endif
+#if FW_PREFETCH == 1
         if (lane == 0 && tile + n_warps < F.n_wtiles) {           // the tile this warp takes next, on its way to L2
             const int64_t nb = (tile + n_warps) * FW_TILE;
             int64_t sz = A.p_end - nb; if (sz > FW_TILE) sz = FW_TILE; sz = (sz + 15) & ~(int64_t)15;
             if (sz > 0) asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(A.bytes_al + nb), "r"((uint32_t)sz) : "memory");
         }
+#elif FW_PREFETCH == 2
+        // on their way to L2: the rest of this tile (its first chunks are loaded right away) and the head of the tile this warp
+        // takes next -- never more than a tile per warp, so that nothing prefetched is evicted before it is used
+        if (lane < 2) {
+            const int64_t nb = lane == 0 ? ts + 2 * WB : (tile + n_warps) * FW_TILE;
+            int64_t sz = A.p_end - nb;
+            const int64_t want = lane == 0 ? FW_TILE - 2 * WB + FW_HALO : 2 * WB;
+            if (sz > want) sz = want;
+            sz = (sz + 15) & ~(int64_t)15;
+            if (sz > 0) asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(A.bytes_al + nb), "r"((uint32_t)sz) : "memory");
+        }
+#endif
 #pragma unroll 1
         for (int64_t r = F.wt_first[tile]; r < A.n_rec; ++r) {
             const int64_t rs = rec_pos(A, r);
@@ -349,29 +383,46 @@ __global__ void __launch_bounds__(FW_WARPS * 32, 3) encode_fasta_kernel(const __
             __syncwarp();
             const uint8_t *const tb = A.bytes_al + ts;
             const int end_rel = A.p_end - ts > (1 << 20) ? (1 << 20) : (int)(A.p_end - ts);
+            const int lim_rel = end_rel;                                         // bytes from here on read as zero
+            uint4 *const stg = sm.stage[warp];
+            if ((sa_rel & ~(WB - 1)) < he_rel) stage_chunk(stg, tb, sa_rel & ~(WB - 1), lim_rel, lane);
 #pragma unroll 1
             for (int c_rel = sa_rel & ~(WB - 1); c_rel < he_rel; c_rel += WB) {
                 const int q_rel = c_rel + lane * LB;                             // tile offset of this lane's first byte
+                // this chunk's bytes arrive from the staging buffer; the next chunk's copy starts before the work on this one
+                asm volatile("cp.async.wait_group 0;" ::: "memory");
                 // ---- interior chunk of wrapped lines (the bulk of a FASTA record): all 2 KiB are body bytes of the piece, lines
                 // are longer than a lane, so each lane holds 64 body bytes and at most one predicted line end.  Streamlined:
                 // no per-byte flags, no masks; falls through to the general code below if any lane fails the layout check ----
                 // The 64 bytes read past the tile's end take the same road with one active lane (nact = active lanes).
                 const int left = he_rel - c_rel;
-                if (d >= 65u && P.fast_lut && nl_skips && c_rel >= sa_rel && (left >= WB || (left & 63) == 0) &&
-                    c_rel + min(left, WB) <= end_rel && yb + c_rel >= 0) {
-                    const int nact = left >= WB ? 32 : left >> 6;
-                    const bool on = lane < nact;
-                    uint4 v[4];
-                    {
-                        const uint4 *src = reinterpret_cast<const uint4 *>(tb + q_rel);
-#pragma unroll
-                        for (int j = 0; j < 4; ++j) v[j] = on ? __ldg(src + j) : make_uint4(0x41414141u, 0x41414141u, 0x41414141u, 0x41414141u);
-                    }
+                const bool lean = d >= 65u && P.fast_lut && nl_skips && c_rel >= sa_rel && (left >= WB || (left & 63) == 0) &&
+                                  c_rel + min(left, WB) <= end_rel && yb + c_rel >= 0;
+                const int nact = left >= WB ? 32 : left >> 6;
+                const bool on = lane < nact;
+                uint32_t tn = 64u;                                               // lane index of the predicted line end (>= 64: none)
+                int u = 0;
+                bool probe_ok = true;
+                if (lean) {
                     const uint32_t c = col_p + ((uint32_t)(yb + q_rel) - y_p);   // column counted from the piece's first line
                     const uint32_t q = dmul ? __umulhi(c, dmul) : (uint32_t)(c >= d);
                     const uint32_t col = c - q * d;
-                    const uint32_t tn = on ? (uint32_t)W - col : 64u;            // lane index of the predicted line end (>= 64: none)
-                    const int u = (int)(q * (uint32_t)W + col) - (int)col_p;
+                    if (on) tn = (uint32_t)W - col;
+                    u = (int)(q * (uint32_t)W + col) - (int)col_p;
+                    if (tn < 64u) {
+                        // the byte where the closed form puts the line end must be '\n'; in the staging buffer it becomes an 'A',
+                        // so that the classification below has one question to ask of all 64 bytes, and its code is deleted later
+                        uint8_t *pb = reinterpret_cast<uint8_t *>(stg + (tn >> 4) * 32 + lane) + (tn & 15u);
+                        probe_ok = *pb == '\n';
+                        *pb = 'A';
+                    }
+                }
+                uint4 v[4];
+#pragma unroll
+                for (int j = 0; j < 4; ++j) v[j] = stg[j * 32 + lane];
+                if (c_rel + WB < he_rel) stage_chunk(stg, tb, c_rel + WB, lim_rel, lane);
+                if (lean) {
+                    if (!on) { v[0] = v[1] = v[2] = v[3] = make_uint4(0x41414141u, 0x41414141u, 0x41414141u, 0x41414141u); }
                     uint32_t C[4], dd[16];
                     {
                         const uint32_t *xw = reinterpret_cast<const uint32_t *>(v);
@@ -380,7 +431,7 @@ __global__ void __launch_bounds__(FW_WARPS * 32, 3) encode_fasta_kernel(const __
                         for (int j = 0; j < 16; ++j) {
                             const uint32_t x = xw[j];
                             cb[j] = (x & 0x06060606u) * 0x00820820u;
-                            const uint32_t m = (x >> 2) & ~(x >> 1) & 0x01010101u;
+                            const uint32_t m = __umulhi(x, mh30) & ~__umulhi(x, mh31) & 0x01010101u;
                             dd[j] = (x & 0xD9D9D9D9u) ^ (m * 0x0fu + 0x41414141u);
                         }
 #pragma unroll
@@ -391,22 +442,10 @@ __global__ void __launch_bounds__(FW_WARPS * 32, 3) encode_fasta_kernel(const __
                             C[h] = ((y & 0x55555555u) << 1) | (((y >> 1) ^ y) & 0x55555555u);
                         }
                     }
-                    const uint32_t a0 = dd[0] | dd[1] | dd[2] | dd[3], a1 = dd[4] | dd[5] | dd[6] | dd[7];
-                    const uint32_t a2 = dd[8] | dd[9] | dd[10] | dd[11], a3 = dd[12] | dd[13] | dd[14] | dd[15];
-                    const uint32_t gsel = tn < 64u ? tn >> 4 : 4u;
-                    const uint32_t other = (gsel == 0u ? 0u : a0) | (gsel == 1u ? 0u : a1) | (gsel == 2u ? 0u : a2) | (gsel == 3u ? 0u : a3);
-                    bool ok = other == 0u;
-                    if (gsel < 4u) {
-                        uint32_t s0 = gsel == 0u ? dd[0] : (gsel == 1u ? dd[4] : (gsel == 2u ? dd[8] : dd[12]));
-                        uint32_t s1 = gsel == 0u ? dd[1] : (gsel == 1u ? dd[5] : (gsel == 2u ? dd[9] : dd[13]));
-                        uint32_t s2 = gsel == 0u ? dd[2] : (gsel == 1u ? dd[6] : (gsel == 2u ? dd[10] : dd[14]));
-                        uint32_t s3 = gsel == 0u ? dd[3] : (gsel == 1u ? dd[7] : (gsel == 2u ? dd[11] : dd[15]));
-                        const uint32_t wi = (tn >> 2) & 3u;
-                        const uint32_t bm = ~(0xffu << (8 * (tn & 3u)));
-                        s0 &= wi == 0u ? bm : 0xffffffffu; s1 &= wi == 1u ? bm : 0xffffffffu;
-                        s2 &= wi == 2u ? bm : 0xffffffffu; s3 &= wi == 3u ? bm : 0xffffffffu;
-                        ok = ok && (s0 | s1 | s2 | s3) == 0u && __ldg(tb + q_rel + tn) == '\n';
-                    }
+                    uint32_t any = 0u;
+#pragma unroll
+                    for (int j = 0; j < 16; ++j) any |= dd[j];
+                    const bool ok = probe_ok && any == 0u;
                     if (__all_sync(FULL, ok)) {
                         int n = 64;
                         if (tn < 64u) {                                          // the line end leaves the code plane
@@ -437,22 +476,21 @@ __global__ void __launch_bounds__(FW_WARPS * 32, 3) encode_fasta_kernel(const __
                         }
                         continue;
                     }
+                    // some byte is not one of ACGT (an N, say): the general code takes the chunk, on the bytes as they are in memory
+                    const uint4 *src = reinterpret_cast<const uint4 *>(tb + q_rel);
+#pragma unroll
+                    for (int j = 0; j < 4; ++j) v[j] = q_rel + 16 * j < lim_rel ? __ldg(src + j) : make_uint4(0, 0, 0, 0);
                 }
                 const int ia = min(max(sa_rel - q_rel, 0), 64), ib = min(max(he_rel - q_rel, 0), 64);   // its bytes [ia, ib) belong to the piece
                 const int64_t ib64 = -(yb + q_rel);                              // first body byte of the record in this lane
                 const int ibody = ib64 <= 0 ? 0 : (ib64 >= 64 ? 64 : (int)ib64);
                 const int i1 = max(ia, ibody);                                   // first body byte of the piece in this lane
                 const bool act = i1 < ib;
-                uint4 v[4];
-                {
-                    const uint4 *src = reinterpret_cast<const uint4 *>(tb + q_rel);
-#pragma unroll
-                    for (int j = 0; j < 4; ++j) v[j] = (act && q_rel + 16 * j < end_rel) ? __ldg(src + j) : make_uint4(0, 0, 0, 0);
-                }
                 // keep mask and kept-base index from the closed form
                 unsigned long long range = 0ull, Kp = 0ull;
                 bool col0 = false;                                               // the piece's first body byte in this lane starts a line
-                int u = 0, tnl = 64;                                             // tnl: lane index of the first predicted newline
+                u = 0;
+                int tnl = 64;                                             // tnl: lane index of the first predicted newline
                 if (act) {
                     range = (i1 == 0 && ib == 64) ? ~0ull : (from_pos(i1) & ~from_pos(ib));
                     const uint32_t y1 = (uint32_t)(yb + q_rel + i1);             // body index of byte i1
