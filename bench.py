@@ -456,6 +456,8 @@ def bench_config(dn, torch, D: Dist, local: int, config: int, k: int, args, *, e
     kern_ms = float(np.median(per_step_ms))
     kname = {"bpe": "bpe_merge_kernel"}.get(tokkw["mode"], "encode_tiles_v7<dense>" if tok.cfg.class_lut is not None
                                                and not tok.cfg.strip_headers else "encode_tiles_v5")
+    if kname == "encode_tiles_v5" and tok.fast_path_taken():
+        kname = "encode_fasta_kernel"                            # the regular-layout encoder served the call (dnatok.h)
     roof = {"bound": "hbm", "kernel": kname, "achieved": alg_bytes / (kern_ms * 1e-3) / 1e9, "peak": peak, "unit": "GB/s",
             "peak_source": peak_src, "algorithmic_bytes_per_launch": alg_bytes,
             "bytes_per_base": alg_bytes / max(1, bases), "kernel_ms": kern_ms,
