@@ -77,6 +77,25 @@ __device__ __forceinline__ int64_t kept_before(int64_t y, int W) {
     return line * W + (col < W ? col : W);
 }
 
+// position of the first '\n' among the bytes al[from, to), or `to` if there is none; al is 16-byte aligned and is read 16 bytes
+// at a time (up to 15 bytes past `to`, like every other kernel here).  A byte equals '\n' iff its XOR with 0x0A is zero; the
+// lowest flag of the classic zero-byte test is exact (a false flag can only sit above a true one).
+__device__ __forceinline__ int64_t find_nl(const uint8_t *al, int64_t from, int64_t to) {
+    for (int64_t p = from & ~(int64_t)15; p < to; p += 16) {
+        const uint4 v = __ldg(reinterpret_cast<const uint4 *>(al + p));
+        const uint32_t w[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const uint32_t y = w[j] ^ 0x0A0A0A0Au;
+            uint32_t z = (y - 0x01010101u) & ~y & 0x80808080u;
+            const int64_t wp = p + 4 * j;
+            if (wp < from) z = from - wp >= 4 ? 0u : z & (0xffffffffu << (8 * (int)(from - wp)));
+            if (z) { const int64_t pos = wp + ((__ffs((int)z) - 1) >> 3); return pos < to ? pos : to; }
+        }
+    }
+    return to;
+}
+
 __global__ void __launch_bounds__(256) fasta_parse_kernel(const __grid_constant__ FastaArgs F) {
     const EncArgs &A = F.e;
     const EncParams &P = A.prm;
@@ -85,10 +104,21 @@ __global__ void __launch_bounds__(256) fasta_parse_kernel(const __grid_constant_
     if (t < F.n_wtiles) {
         // last record whose start is at or before the tile's first byte (0 if the tile starts in front of every record)
         const int64_t pos = t * FW_TILE;
-        int64_t lo = 0, hi = A.n_rec + 1;                       // number of offsets <= pos
+        // number of offsets <= pos, by a 16-way search: the 16 probes of a step are independent loads, so the chain of
+        // dependent memory round trips is log16 instead of log2 of the record count
+        int64_t lo = 0, hi = A.n_rec + 1;                       // every m < lo has offset <= pos, no m >= hi has
         while (lo < hi) {
-            const int64_t mid = (lo + hi) >> 1;
-            if (rec_pos(A, mid) <= pos) lo = mid + 1; else hi = mid;
+            const int64_t step = (hi - lo + 15) >> 4;
+            bool le[16];
+#pragma unroll
+            for (int i = 0; i < 16; ++i) { const int64_t m = lo + i * step; le[i] = m < hi && rec_pos(A, m) <= pos; }
+            int c = 0;
+#pragma unroll
+            for (int i = 0; i < 16; ++i) c += le[i] ? 1 : 0;    // the probes that hold form a prefix (offsets ascend)
+            if (c == 0) { hi = lo; break; }
+            const int64_t nhi = lo + c * step;                  // the first probe that fails, if one was made
+            lo = lo + (c - 1) * step + 1;
+            if (c < 16 && nhi < hi) hi = nhi;
         }
         F.wt_first[t] = (int32_t)(lo > 0 ? lo - 1 : 0);
     }
@@ -96,24 +126,24 @@ __global__ void __launch_bounds__(256) fasta_parse_kernel(const __grid_constant_
     const int64_t a = rec_pos(A, t), e = rec_pos(A, t + 1), L = e - a;
     const uint8_t *b = A.bytes_al + a;
     bool bad = L >= (1ll << 31);
+    const uint32_t last_byte = L > 0 ? (uint32_t)__ldg(b + L - 1) : 0u;     // asked for early: a cache line of its own
+    const bool nl_skipped = __ldg(F.e.lut + (uint8_t)'\n') == CLS_SKIP;
     int64_t B = 0;
     if (P.strip_headers && L > 0 && b[0] == '>') {
-        int64_t i = 1;
         const int64_t lim = L < FW_HDR_BOUND ? L : FW_HDR_BOUND;
-        while (i < lim && b[i] != '\n') ++i;
+        const int64_t i = find_nl(A.bytes_al, a + 1, a + lim) - a;
         if (i < lim) B = i + 1;                                 // through the '\n'
         else if (lim == L) B = L;                               // a header with no line end runs to the record's end (Q4)
         else bad = true;
     }
     // a record's last line is usually shorter than the others: its line end, the record's last byte, is set apart
     int64_t Z = 0;
-    if (L - B > 0 && b[L - 1] == '\n' && F.e.lut[(uint8_t)'\n'] == CLS_SKIP) Z = 1;
+    if (L - B > 0 && last_byte == '\n' && nl_skipped) Z = 1;
     const int64_t body = L - B - Z;
     int64_t W = body;                                           // one line without a line end
     if (body > 0) {
-        int64_t i = 0;
         const int64_t lim = body < FW_LINE_BOUND ? body : FW_LINE_BOUND;
-        while (i < lim && b[B + i] != '\n') ++i;
+        const int64_t i = find_nl(A.bytes_al, a + B, a + B + lim) - (a + B);
         if (i < lim) W = i;
         // (else: a long single line; the encode kernel checks that it holds no line end)
     }
