@@ -61,11 +61,18 @@ struct SmemFa {
 // read as zero.  One cp.async group per chunk.
 __device__ __forceinline__ void stage_chunk(uint4 *stg, const uint8_t *tb, int c, int lim, int lane) {
     const int q = c + lane * LB;
+    const uint32_t dst = (uint32_t)__cvta_generic_to_shared(stg + lane);
+    const uint8_t *src = tb + q;
+    if (c + WB <= lim) {                                         // the whole chunk lies inside the input (warp-uniform)
 #pragma unroll
-    for (int j = 0; j < 4; ++j) {
-        const uint32_t dst = (uint32_t)__cvta_generic_to_shared(stg + j * 32 + lane);
-        const int sz = q + 16 * j < lim ? 16 : 0;
-        asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(dst), "l"(tb + q + 16 * j), "r"(sz) : "memory");
+        for (int j = 0; j < 4; ++j)
+            asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst + j * 512), "l"(src + 16 * j) : "memory");
+    } else {
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const int sz = q + 16 * j < lim ? 16 : 0;
+            asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(dst + j * 512), "l"(src + 16 * j), "r"(sz) : "memory");
+        }
     }
     asm volatile("cp.async.commit_group;" ::: "memory");
 }
@@ -209,7 +216,8 @@ __global__ void __launch_bounds__(OS_NT) offsets_scan_kernel(const int32_t *tok,
 }
 
 // ---- emission from a warp's private stream (code words cw, flag words fw; base u at bits 31-2(u&15).. of cw[u>>4]) ----
-template <typename IdT, int K, bool SINGLE, bool REMAP>
+// FLAGS = false: the caller knows that no base of the piece is flagged (the flag words are not read)
+template <typename IdT, int K, bool SINGLE, bool REMAP, bool FLAGS = true>
 __device__ __forceinline__ void emit_group_w(const EncArgs &A, const uint32_t *cw, const uint32_t *fw, int o, IdT *dst, bool affine) {
     constexpr int R = 16 / (int)sizeof(IdT);
     constexpr int W = 2 * K;
@@ -228,7 +236,7 @@ __device__ __forceinline__ void emit_group_w(const EncArgs &A, const uint32_t *c
         for (int i = 0; i < NA; ++i) a[i] = __funnelshift_l(raw[i + 1], raw[i], s);
     }
     uint32_t anybad = 0;
-    {
+    if (FLAGS) {
         const int w = o >> 5, s = o & 31;
         uint32_t raw[NF + 1];
 #pragma unroll
@@ -250,7 +258,7 @@ __device__ __forceinline__ void emit_group_w(const EncArgs &A, const uint32_t *c
         if (SINGLE) id[t] = affine ? P.nt_ids[0] + (int32_t)c[t] : P.nt_ids[c[t]];
         else id[t] = (REMAP && P.remap4) ? __ldg(P.remap4 + c[t]) : P.base_id + (int32_t)c[t];
     }
-    if (anybad) {
+    if (FLAGS && anybad) {
 #pragma unroll
         for (int t = 0; t < R; ++t) {
             const int bo = K * t, i = bo >> 5, s = bo & 31;
@@ -296,9 +304,13 @@ __device__ __forceinline__ int32_t w_window_id(const EncParams &P, const uint32_
 }
 
 template <typename IdT, int KK>
-__device__ __forceinline__ void emit_group_sel(const EncArgs &A, const uint32_t *cw, const uint32_t *fw, int u, IdT *dst, bool affine, int kk) {
+__device__ __forceinline__ void emit_group_sel(const EncArgs &A, const uint32_t *cw, const uint32_t *fw, int u, IdT *dst, bool affine, int kk,
+                                               bool flags) {
     if constexpr (KK == 0) emit_group_w<IdT, 1, true, false>(A, cw, fw, u, dst, affine);
-    else if constexpr (KK > 0) emit_group_w<IdT, KK, false, false>(A, cw, fw, u, dst, false);
+    else if constexpr (KK > 0) {
+        if (flags) emit_group_w<IdT, KK, false, false, true>(A, cw, fw, u, dst, false);
+        else emit_group_w<IdT, KK, false, false, false>(A, cw, fw, u, dst, false);
+    }
     else switch (kk) {
         case 0: emit_group_w<IdT, 1, true, false>(A, cw, fw, u, dst, affine); break;
         case 1: emit_group_w<IdT, 1, false, true>(A, cw, fw, u, dst, false); break;
@@ -412,7 +424,19 @@ __global__ void __launch_bounds__(FW_WARPS * 32, 3) encode_fasta_kernel(const __
             const int end_rel = A.p_end - ts > (1 << 20) ? (1 << 20) : (int)(A.p_end - ts);
             const int lim_rel = end_rel;                                         // bytes from here on read as zero
             uint4 *const stg = sm.stage[warp];
+            bool has_flags = false;
             if ((sa_rel & ~(WB - 1)) < he_rel) stage_chunk(stg, tb, sa_rel & ~(WB - 1), lim_rel, lane);
+            // chunks [lean_lo, lean_hi) of the piece may take the lean road below: whole chunks of body bytes inside the input
+            // (lean_hi: the last one may be the 64-byte multiple read past the tile's end)
+            int lean_lo = 1 << 30, lean_hi = 0;
+            if (d >= 65u && P.fast_lut && nl_skips) {
+                lean_lo = (sa_rel + WB - 1) & ~(WB - 1);
+                if (yb + lean_lo < 0) lean_lo = (int)((-yb + WB - 1) & ~(int64_t)(WB - 1));
+                const int full_end = min(he_rel, end_rel) & ~(WB - 1);            // end of the last whole chunk
+                lean_hi = full_end;
+                const int rest = he_rel - full_end;
+                if (rest > 0 && (rest & 63) == 0 && he_rel <= end_rel) lean_hi = full_end + WB;
+            }
 #pragma unroll 1
             for (int c_rel = sa_rel & ~(WB - 1); c_rel < he_rel; c_rel += WB) {
                 const int q_rel = c_rel + lane * LB;                             // tile offset of this lane's first byte
@@ -423,8 +447,7 @@ __global__ void __launch_bounds__(FW_WARPS * 32, 3) encode_fasta_kernel(const __
                 // no per-byte flags, no masks; falls through to the general code below if any lane fails the layout check ----
                 // The 64 bytes read past the tile's end take the same road with one active lane (nact = active lanes).
                 const int left = he_rel - c_rel;
-                const bool lean = d >= 65u && P.fast_lut && nl_skips && c_rel >= sa_rel && (left >= WB || (left & 63) == 0) &&
-                                  c_rel + min(left, WB) <= end_rel && yb + c_rel >= 0;
+                const bool lean = c_rel >= lean_lo && c_rel < lean_hi;
                 const int nact = left >= WB ? 32 : left >> 6;
                 const bool on = lane < nact;
                 uint32_t tn = 64u;                                               // lane index of the predicted line end (>= 64: none)
@@ -624,6 +647,7 @@ __global__ void __launch_bounds__(FW_WARPS * 32, 3) encode_fasta_kernel(const __
                 else if (n == 63) v7::delete_one(C, bad, __clzll((long long)~keep));
                 else if (n != 64) v7::delete_runs(C, bad, keep);
                 const uint32_t Fw[2] = {(uint32_t)(bad >> 32), (uint32_t)bad};
+                if (__any_sync(FULL, bad != 0ull)) has_flags = true;             // (warp-uniform) the piece holds flagged bases
                 // append at the closed-form position u
                 if (__all_sync(FULL, n >= 32)) {
                     // every lane fills a whole word: interior words are written once (a lane's last partial word travels to the
@@ -689,7 +713,7 @@ __global__ void __launch_bounds__(FW_WARPS * 32, 3) encode_fasta_kernel(const __
                 if (nwp < xa || xb <= xa) { xa = nwp; xb = nwp; }
             }
             for (int x = xa + lane * R; x < xb; x += 32 * R)
-                emit_group_sel<IdT, KK>(A, cw, fw, ufirst + x * k, idp + x, affine, kk);
+                emit_group_sel<IdT, KK>(A, cw, fw, ufirst + x * k, idp + x, affine, kk, has_flags);
             {
                 // the windows in front of and behind the groups, one per lane
                 const int n1 = xa, n2 = nwp - xb;
