@@ -355,8 +355,9 @@ __global__ void __launch_bounds__(FW_WARPS * 32, 3) encode_fasta_kernel(const __
     const uint32_t mh31 = 0x80000000u | (uint32_t)(F.n_wtiles < 0), mh30 = mh31 >> 1;
 
     // Tiles are handed out through a counter (F.irregular + 2, zeroed with the flag): the first one of a warp is its own index,
-    // every later one is taken when the warp starts the tile before it, so that a warp always knows its next tile (whose head it
-    // prefetches) and no SM is left idle while others still have several tiles of uneven cost in front of them.
+    // every later one is taken when the warp starts the tile before it, so that no SM is left idle while others still have
+    // several tiles of uneven cost in front of them.  (No L2 prefetch: with the next chunk always in flight it bought no time
+    // and cost a fifth more DRAM reads.)
     const int64_t n_warps = (int64_t)gridDim.x * FW_WARPS;
     unsigned long long *const tile_ctr = reinterpret_cast<unsigned long long *>(F.irregular + 2);
     int64_t tile = (int64_t)blockIdx.x * FW_WARPS + warp;
@@ -367,16 +368,6 @@ __global__ void __launch_bounds__(FW_WARPS * 32, 3) encode_fasta_kernel(const __
         next_tile = __shfl_sync(FULL, next_tile, 0);
         const int64_t ts = tile * FW_TILE, te = ts + FW_TILE < A.p_end ? ts + FW_TILE : A.p_end;
         int nseg = 0;
-        // on their way to L2: the rest of this tile (its first chunks are loaded right away) and the head of the tile this warp
-        // takes next -- never more than a tile per warp, so that nothing prefetched is evicted before it is used
-        if (lane < 2) {
-            const int64_t nb = lane == 0 ? ts + 2 * WB : next_tile * FW_TILE;
-            int64_t sz = A.p_end - nb;
-            const int64_t want = lane == 0 ? FW_TILE - 2 * WB + FW_HALO : 2 * WB;
-            if (sz > want) sz = want;
-            sz = (sz + 15) & ~(int64_t)15;
-            if (sz > 0) asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(A.bytes_al + nb), "r"((uint32_t)sz) : "memory");
-        }
 #pragma unroll 1
         for (int64_t r = F.wt_first[tile]; r < A.n_rec; ++r) {
             const int64_t rs = rec_pos(A, r);
