@@ -44,7 +44,8 @@ static_assert(FW_WORDS % 4 == 0, "per-warp streams stay 16-byte aligned");
 struct FastaArgs {
     EncArgs e;
     int32_t *par;                // [n_rec][4]: B (bytes of the header line, 0 if none), W (line width; >= 1), Z (1: the record's
-                                 //             last byte is the line end of its last line)
+                                 //             last byte is the line end of its last line), dmul (floor(2^32 / (W + 1)) + 1, or 0
+                                 //             if W + 1 > 65536)
     int32_t *rec_tok;            // [n_rec] tokens of every record
     int32_t *wt_first;           // [n_wtiles] record that holds the tile's first byte (first record starting behind it if none)
     uint32_t *irregular;         // set when the input does not have the regular layout
@@ -156,7 +157,9 @@ __global__ void __launch_bounds__(256) fasta_parse_kernel(const __grid_constant_
     }
     if (W < 1) { W = 1; if (body > 0) bad = true; }             // a body that starts with an empty line is not regular
     if (bad) { *F.irregular = 1u; B = 0; W = 1; Z = 0; }
-    F.par[4 * t] = (int32_t)B; F.par[4 * t + 1] = (int32_t)(W > 0x7fffffff ? 0x7fffffff : W); F.par[4 * t + 2] = (int32_t)Z;
+    const int64_t Wc = W > 0x7fffffff ? 0x7fffffff : W, dd = Wc + 1;
+    const uint32_t dmul = dd <= 65536 ? (uint32_t)(0x100000000ull / (unsigned long long)dd) + 1u : 0u;    // see div_d below
+    reinterpret_cast<int4 *>(F.par)[t] = make_int4((int32_t)B, (int32_t)Wc, (int32_t)Z, (int32_t)dmul);
     const int64_t n = bad ? 0 : kept_before(body, (int)W);
     int64_t tok = n;
     if (P.mode == MODE_KMER) { const int64_t q = n / P.k; tok = q + tail_tokens((int)(n - q * P.k), P); }
@@ -323,6 +326,15 @@ __device__ __forceinline__ void emit_group_sel(const EncArgs &A, const uint32_t 
     }
 }
 
+// y / d for any 32-bit y by one multiply-high and a correction: with dmul = floor(2^32 / d) + 1 the estimate is the quotient or
+// one more (y dmul / 2^32 = y / d + y e / (d 2^32), e = dmul d - 2^32 <= d).  dmul == 0 (d > 65536): the division itself.
+__device__ __forceinline__ uint32_t div_d(uint32_t y, uint32_t d, uint32_t dmul) {
+    if (dmul == 0u) return y / d;
+    uint32_t q = __umulhi(y, dmul);
+    if (q * d > y) --q;
+    return q;
+}
+
 __device__ __forceinline__ int clamp64(int64_t v) { return v < 0 ? 0 : (v > 64 ? 64 : (int)v); }
 
 // ======================================================================================================
@@ -376,11 +388,12 @@ __global__ void __launch_bounds__(FW_WARPS * 32, 3) encode_fasta_kernel(const __
             const int64_t sa = rs > ts ? rs : ts, sb = re < te ? re : te;       // the record's piece inside this tile
             if (sb <= sa) continue;
             if (++nseg > FW_MAXSEG) { irregular = true; break; }
-            const int B = __ldg(F.par + 4 * r), W = __ldg(F.par + 4 * r + 1), Z = __ldg(F.par + 4 * r + 2);
+            const int4 par = __ldg(reinterpret_cast<const int4 *>(F.par) + r);
+            const int B = par.x, W = par.y, Z = par.z;
             const uint32_t d = (uint32_t)W + 1u;
             // c / d in one multiply for the columns c < d + FW_TILE + FW_HALO met below: exact while c * (dmul * d - 2^32) < 2^32
             // (every d up to 2^14) or c < 2 d - 1 (the larger d)
-            const uint32_t dmul = d <= 65536u ? (uint32_t)(0x100000000ull / d) + 1u : 0u;
+            const uint32_t dmul = (uint32_t)par.w;
             const int64_t bend = re - Z;                                         // end of the body (the record's final line end set apart)
             const int64_t sbb = sb < bend ? sb : bend;
             // everything below is 32 bits wide and relative to the tile's first byte
@@ -388,22 +401,22 @@ __global__ void __launch_bounds__(FW_WARPS * 32, 3) encode_fasta_kernel(const __
             int64_t he = sb;                                                     // bytes behind a piece that ends at the tile's end:
             if (sb == te && re > sb) { he = sb + FW_HALO; if (he > A.p_end) he = A.p_end; }   //   the windows that start in the piece run into them
             if (he > bend) he = bend;
-            const int he_rel = (int)(he - ts);
+            int he_rel = (int)(he - ts);
             const int64_t yb = ts - rs - B;                                      // body index of the tile's first byte (may be negative)
             // body index, line and column of the piece's first body byte; bases of the record in front of / through the piece
             const uint32_t y_p = (uint32_t)(sa - rs > B ? sa - rs - B : 0);
-            const uint32_t line_p = y_p / d, col_p = y_p - line_p * d;
+            const uint32_t line_p = div_d(y_p, d, dmul), col_p = y_p - line_p * d;
             // (a record is shorter than 2^31 bytes -- the parse kernel flags anything longer -- so base counts fit 32 bits)
             const uint32_t K0 = line_p * (uint32_t)W + col_p;
             const uint32_t y_e = (uint32_t)(sbb - rs > B ? sbb - rs - B : 0);
-            const uint32_t line_e = y_e / d, col_e = y_e - line_e * d;
+            const uint32_t line_e = div_d(y_e, d, dmul), col_e = y_e - line_e * d;
             const int nK = (int)(line_e * (uint32_t)W + col_e - K0);             // bases of the piece
             // windows of the record: only matters when the record ends near the piece
             constexpr uint32_t FAR = 0xffffffffu;
             uint32_t nwin = FAR, n_r = FAR;
             if (re - sb < 2 * FW_HALO) {
                 const uint32_t y_r = (uint32_t)(bend - rs > B ? bend - rs - B : 0);
-                const uint32_t line_r = y_r / d, col_r = y_r - line_r * d;
+                const uint32_t line_r = div_d(y_r, d, dmul), col_r = y_r - line_r * d;
                 n_r = line_r * (uint32_t)W + col_r;
                 nwin = n_r / (uint32_t)k;
             }
@@ -416,6 +429,40 @@ __global__ void __launch_bounds__(FW_WARPS * 32, 3) encode_fasta_kernel(const __
             const int lim_rel = end_rel;                                         // bytes from here on read as zero
             uint4 *const stg = sm.stage[warp];
             bool has_flags = false;
+            // ---- the bytes behind a piece that ends at the tile's end.  Only the k - 1 <= 14 bases that the piece's last windows
+            // run into are needed, and the warp that owns the next tile is the one that checks them.  Wrapped lines of ACGT: 16
+            // bytes, classified by every lane alike, at most one predicted line end dropped, appended by lane 0 at stream
+            // position nK.  Anything else (an N among them, a header, short lines) goes through the chunk loop below. ----
+            if (he - sb >= 16 && d >= 65u && P.fast_lut && nl_skips && yb + (sb - ts) >= 0) {
+                const int sb_rel = (int)(sb - ts);
+                const uint4 hv = __ldg(reinterpret_cast<const uint4 *>(tb + sb_rel));
+                const uint32_t c = col_p + ((uint32_t)(yb + sb_rel) - y_p);
+                const uint32_t q = dmul ? __umulhi(c, dmul) : (uint32_t)(c >= d);
+                const uint32_t tn = (uint32_t)W - (c - q * d);                    // offset of the predicted line end (>= 16: none here)
+                const uint32_t xw[4] = {hv.x, hv.y, hv.z, hv.w};
+                uint32_t cb[4], inval = 0u;
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                    const uint32_t x = xw[j];
+                    cb[j] = (x & 0x06060606u) * 0x00820820u;
+                    const uint32_t m = (x >> 2) & ~(x >> 1) & 0x01010101u;
+                    uint32_t dj = (x & 0xD9D9D9D9u) ^ (m * 0x0fu + 0x41414141u);
+                    if ((tn >> 2) == (uint32_t)j) dj &= ~(0xffu << (8 * (tn & 3u)));
+                    inval |= dj;
+                }
+                if (inval == 0u) {
+                    const uint32_t lo2 = __byte_perm(cb[0], cb[1], 0x0073), hi2 = __byte_perm(cb[2], cb[3], 0x0073);
+                    const uint32_t y = __brev(__byte_perm(lo2, hi2, 0x5410));
+                    uint32_t C = ((y & 0x55555555u) << 1) | (((y >> 1) ^ y) & 0x55555555u);
+                    if (tn < 16u) { const uint32_t T = ~(0xffffffffu >> (2 * tn)); C = (C & T) | ((C << 2) & ~T); }
+                    if (lane == 0) {
+                        const int sh = 2 * (nK & 15);
+                        atomicOr(&cw[nK >> 4], C >> sh);
+                        if (sh) atomicOr(&cw[(nK >> 4) + 1], C << (32 - sh));
+                    }
+                    he_rel = sb_rel;                                             // the chunk loop stops at the tile's end
+                }
+            }
             if ((sa_rel & ~(WB - 1)) < he_rel) stage_chunk(stg, tb, sa_rel & ~(WB - 1), lim_rel, lane);
             // chunks [lean_lo, lean_hi) of the piece may take the lean road below: whole chunks of body bytes inside the input
             // (lean_hi: the last one may be the 64-byte multiple read past the tile's end)
