@@ -374,9 +374,10 @@ def bench_config(dn, torch, D: Dist, local: int, config: int, k: int, args, *, e
         mask = torch.empty((n_rec, L), dtype=torch.uint8, device="cuda")
 
     def step():
-        tok.encode(d_bytes, d_off, ids_out=ids, out_offsets=out_off)
-        if L:
-            tok.pad(ids, out_off, batch_ids=batch, mask=mask)
+        if L:       # dnatok_encode_pad: steps 1-6 in one call; regular layouts go straight into the batch (no CSR ids in HBM)
+            tok.encode_padded(d_bytes, d_off, ids_out=ids, out_offsets=out_off, batch_ids=batch, mask=mask)
+        else:
+            tok.encode(d_bytes, d_off, ids_out=ids, out_offsets=out_off)
 
     # ---- device-timed region: K steps, CUDA events on the launching (current) stream ---------------------------------
     for _ in range(max(args.warmup, 3)):
@@ -423,8 +424,13 @@ def bench_config(dn, torch, D: Dist, local: int, config: int, k: int, args, *, e
         if args.full_parity or config != 5:
             want_ids, want_off = oracle_run(data, offsets, ocfg, host_cores(), want="all")
             ok = bool(np.array_equal(off_h, want_off))
-            ok = ok and bool(np.array_equal(ids[: n_tokens].cpu().numpy().astype(np.int32), want_ids))
-            what = f"every id ({n_tokens}) and every out_offsets entry ({n_rec + 1})"
+            if L and tok.fast_path_taken():                      # fused call: the ids went straight into the batch
+                wb, wm = oracle.pad(want_ids, want_off, ocfg)
+                ok = ok and bool(np.array_equal(batch.cpu().numpy(), wb)) and bool(np.array_equal(mask.cpu().numpy(), wm))
+                what = f"every batch and mask entry ({n_rec} x {L}) and every out_offsets entry ({n_rec + 1})"
+            else:
+                ok = ok and bool(np.array_equal(ids[: n_tokens].cpu().numpy().astype(np.int32), want_ids))
+                what = f"every id ({n_tokens}) and every out_offsets entry ({n_rec + 1})"
             del want_ids
         else:
             # config 5 (10.7 GB of rows): every out_offsets entry, and ids + batch row + mask of 64 sampled records
@@ -432,17 +438,20 @@ def bench_config(dn, torch, D: Dist, local: int, config: int, k: int, args, *, e
             ok = bool(np.array_equal(off_h, want_off))
             rng = np.random.default_rng(1234)
             pick = np.unique(np.concatenate([[0, n_rec - 1], rng.integers(0, n_rec, size=62)]))
+            ids_written = not (L and tok.fast_path_taken())             # the fused call leaves the CSR ids unwritten
             for r in pick:
                 a, b = int(offsets[r]), int(offsets[r + 1])
                 want, _ = oracle.encode(data[a:b], np.array([0, b - a], dtype=np.int64), ocfg)
                 lo = int(want_off[r])
-                got = ids[lo: lo + want.size].cpu().numpy().astype(np.int32)
-                ok = ok and bool(np.array_equal(got, want))
+                if ids_written:
+                    got = ids[lo: lo + want.size].cpu().numpy().astype(np.int32)
+                    ok = ok and bool(np.array_equal(got, want))
                 if L:
                     wb, wm = oracle.pad(want, np.array([0, want.size], dtype=np.int64), ocfg)
                     ok = ok and bool(np.array_equal(batch[r].cpu().numpy(), wb[0]))
                     ok = ok and bool(np.array_equal(mask[r].cpu().numpy(), wm[0]))
-            what = f"every out_offsets entry ({n_rec + 1}) and ids, batch row and mask of {pick.size} sampled records"
+            what = (f"every out_offsets entry ({n_rec + 1}) and " + ("ids, " if ids_written else "") +
+                    f"batch row and mask of {pick.size} sampled records")
         parity_s = ("bit-exact: " + what) if ok else ("MISMATCH: " + what)
 
     # ---- roofline: the method's own bytes over the median step -----------------------------------------------------
@@ -464,8 +473,11 @@ def bench_config(dn, torch, D: Dist, local: int, config: int, k: int, args, *, e
             "traffic": args.traffic if args.traffic is not None else committed_profile(f"config{config}")}
     roof["frac"] = roof["achieved"] / peak
     if L:
-        roof["note"] = ("method bytes only: input + batch_ids + mask; the CSR ids the pad kernel re-reads (%d B written, "
-                        "%d B read per step) are not counted" % (n_tokens * idsz, n_tokens * idsz))
+        if kname == "encode_fasta_kernel":
+            roof["note"] = "method bytes: input + batch_ids + mask; dnatok_encode_pad wrote the tokens straight into the batch (no CSR ids)"
+        else:
+            roof["note"] = ("method bytes only: input + batch_ids + mask; the CSR ids the pad kernel re-reads (%d B written, "
+                            "%d B read per step) are not counted" % (n_tokens * idsz, n_tokens * idsz))
     if tokkw["mode"] == "bpe":
         # the merge loop is bound by instruction issue, not by HBM (SURVEY.md section 7 hard part 5)
         sm_mhz = clk.get("sm_mhz") or 1965.0

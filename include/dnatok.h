@@ -132,6 +132,18 @@ int dnatok_encode(dnatok_t *h, const uint8_t *d_bytes, int64_t n_bytes,
 int dnatok_pad(dnatok_t *h, const void *d_ids, const int64_t *d_out_offsets, int64_t n_records,
                int32_t *d_batch_ids, uint8_t *d_mask, void *stream);
 
+/*
+ * dnatok_encode_pad: steps 1-6 in one call (PAPER.md:84 bytes path through PAPER.md:124-129 padding): d_out_offsets,
+ * d_batch_ids and d_mask end up exactly as after dnatok_encode followed by dnatok_pad with the same arguments.  Inputs laid
+ * out as wrapped FASTA or one line per record (see dnatok_set_fast_path) have their tokens written straight into the batch:
+ * the CSR ids never travel through HBM, and d_ids_out is then left untouched.  Any other input is encoded into d_ids_out and
+ * padded from there.  So d_ids_out / ids_capacity must be given as for dnatok_encode (workspace for the second case), but
+ * the caller may rely on its contents only after dnatok_encode.  EINVAL if the handle has seq_len == 0.  Enqueue only.
+ */
+int dnatok_encode_pad(dnatok_t *h, const uint8_t *d_bytes, int64_t n_bytes, const int64_t *d_rec_offsets,
+                      int64_t n_records, void *d_ids_out, int64_t ids_capacity, int64_t *d_out_offsets,
+                      int32_t *d_batch_ids, uint8_t *d_mask, void *stream);
+
 /* One delivered batch of dnatok_stream_encode (device pointers valid until the callback's stream work ends). */
 typedef struct {
     int64_t first_record;        /* index of the first record in this batch                     */

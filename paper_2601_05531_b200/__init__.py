@@ -24,7 +24,7 @@ from . import _build
 __all__ = [
     "DNATok", "Config", "Batch", "DNATokError", "lib", "library_path",
     "SINGLE_NT", "KMER", "BPE", "I16", "I32", "TAIL_PER_BASE", "TAIL_DROP", "TAIL_UNK", "PAD_LEFT", "PAD_RIGHT",
-    "dnatok_create", "dnatok_destroy", "dnatok_encode", "dnatok_pad", "dnatok_stream_encode", "dnatok_check",
+    "dnatok_create", "dnatok_destroy", "dnatok_encode", "dnatok_pad", "dnatok_encode_pad", "dnatok_stream_encode", "dnatok_check",
     "dnatok_last_error", "dnatok_launch_count", "dnatok_version", "dnatok_config_default", "dnatok_set_super_tile", "dnatok_set_grid_cap", "dnatok_set_fast_path", "dnatok_fast_path_taken",
     "dnatok_stream_encode_from", "dnatok_revcomp", "dnatok_decode", "dnatok_microbatch_rows", "dnatok_embed", "dnatok_widen_ids",
 ]
@@ -102,6 +102,8 @@ def lib() -> ctypes.CDLL:
         L.dnatok_encode.argtypes = [vp, vp, i64, vp, i64, vp, i64, vp, vp]
         L.dnatok_pad.restype = ctypes.c_int
         L.dnatok_pad.argtypes = [vp, vp, vp, i64, vp, vp, vp]
+        L.dnatok_encode_pad.restype = ctypes.c_int
+        L.dnatok_encode_pad.argtypes = [vp, vp, i64, vp, i64, vp, i64, vp, vp, vp, vp]
         L.dnatok_stream_encode.restype = ctypes.c_int
         L.dnatok_stream_encode.argtypes = [vp, vp, i64, vp, i64, i64, ctypes.c_int, i64, _BATCH_FN, vp]
         L.dnatok_stream_encode_from.restype = ctypes.c_int
@@ -171,6 +173,12 @@ def dnatok_encode(h: int, d_bytes: int, n_bytes: int, d_rec_offsets: int, n_reco
 def dnatok_pad(h: int, d_ids: int, d_out_offsets: int, n_records: int, d_batch_ids: int, d_mask: int,
                stream: int = 0) -> None:
     _chk(h, lib().dnatok_pad(h, d_ids, d_out_offsets, n_records, d_batch_ids, d_mask, stream))
+
+
+def dnatok_encode_pad(h: int, d_bytes: int, n_bytes: int, d_rec_offsets: int, n_records: int, d_ids_out: int,
+                      ids_capacity: int, d_out_offsets: int, d_batch_ids: int, d_mask: int, stream: int = 0) -> None:
+    _chk(h, lib().dnatok_encode_pad(h, d_bytes, n_bytes, d_rec_offsets, n_records, d_ids_out, ids_capacity,
+                                    d_out_offsets, d_batch_ids, d_mask, stream))
 
 
 def dnatok_stream_encode(h: int, h_pinned: int, n_bytes: int, h_rec_offsets: int, n_records: int,
@@ -389,9 +397,26 @@ class DNATok:
                    self._stream(stream))
         return batch_ids, mask
 
-    def encode_padded(self, d_bytes, d_rec_offsets, stream=None):
-        ids, off = self.encode(d_bytes, d_rec_offsets, stream=stream)
-        return self.pad(ids, off, stream=stream)
+    def encode_padded(self, d_bytes, d_rec_offsets, ids_out=None, out_offsets=None, batch_ids=None, mask=None, stream=None):
+        """Steps 1-6 in one call -> (batch_ids, mask, out_offsets); the same results as encode() + pad().  ids_out is
+        workspace: regular-layout inputs are written straight into the batch and leave it untouched (dnatok.h)."""
+        t = self._torch
+        assert d_bytes.is_cuda and d_bytes.dtype == t.uint8 and d_bytes.is_contiguous()
+        assert d_rec_offsets.is_cuda and d_rec_offsets.dtype == t.int64 and d_rec_offsets.is_contiguous()
+        n_bytes, n_rec = d_bytes.numel(), d_rec_offsets.numel() - 1
+        L = self.cfg.seq_len
+        if ids_out is None:
+            ids_out = t.empty(max(n_bytes, 1), dtype=self.id_torch_dtype, device=d_bytes.device)
+        if out_offsets is None:
+            out_offsets = t.empty(n_rec + 1, dtype=t.int64, device=d_bytes.device)
+        if batch_ids is None:
+            batch_ids = t.empty((n_rec, L), dtype=t.int32, device=d_bytes.device)
+        if mask is None:
+            mask = t.empty((n_rec, L), dtype=t.uint8, device=d_bytes.device)
+        assert ids_out.dtype == self.id_torch_dtype and out_offsets.dtype == t.int64
+        dnatok_encode_pad(self.h, d_bytes.data_ptr(), n_bytes, d_rec_offsets.data_ptr(), n_rec, ids_out.data_ptr(),
+                          ids_out.numel(), out_offsets.data_ptr(), batch_ids.data_ptr(), mask.data_ptr(), self._stream(stream))
+        return batch_ids, mask, out_offsets
 
     def _batch_cb(self, on_batch):
         cfg = self.cfg

@@ -295,10 +295,17 @@ void launch_strip(const EncArgs &a, int kk, int grid, cudaStream_t st, bool chai
     }
 }
 
+int pad_on(dnatok_t *h, const void *d_ids, const int64_t *d_out_off, int64_t n_rec, int32_t *d_batch,
+           uint8_t *d_mask, cudaStream_t st, int64_t ids_cap, const uint32_t *run_if);
+
+// d_batch != nullptr asks for the padded batch as well (handle with seq_len > 0).  If the regular-layout encoder takes the call
+// it writes the tokens straight into the batch (*fused = true: batch and mask are complete when the launches below have run,
+// whichever encoder ends up serving the call); otherwise *fused stays false and the caller runs the pad kernel on the ids.
 template <typename IdT>
 int launch_tiles(dnatok_t *h, EncCtx &c, const EncParams &prm, const uint8_t *d_bytes, int64_t n_bytes,
                  const int64_t *d_rec_off, int64_t n_rec, int64_t off_bias, void *ids, int64_t ids_cap,
-                 int64_t *out_off, cudaStream_t st) {
+                 int64_t *out_off, cudaStream_t st, int32_t *d_batch = nullptr, uint8_t *d_mask = nullptr,
+                 bool *fused = nullptr) {
     EncArgs a;
     uintptr_t addr = reinterpret_cast<uintptr_t>(d_bytes);
     a.mis = (int64_t)(addr & 15);
@@ -337,6 +344,7 @@ int launch_tiles(dnatok_t *h, EncCtx &c, const EncParams &prm, const uint8_t *d_
         launch_dense<IdT>(a, kk, grid, st);
     } else {
         bool chained = false;                                 // the kernels below follow kernels of this call
+        bool f_fused = false;
         c.fa_tried = false;
         if ((h->fast_path == 2 || (h->fast_path == 1 && n_bytes >= (4ll << 20))) && n_rec < (1ll << 31)) {
             // regular-layout fast path first (encode_fasta.cuh); the chained-scan encoder behind it runs only if the layout
@@ -350,18 +358,34 @@ int launch_tiles(dnatok_t *h, EncCtx &c, const EncParams &prm, const uint8_t *d_
             fa::FastaArgs f;
             f.e = a; f.par = c.fa_par; f.rec_tok = c.fa_tok; f.wt_first = c.fa_first; f.irregular = c.fa_flag;
             f.n_wtiles = (int32_t)n_wtiles;
+            const bool fuse = d_batch != nullptr && fused != nullptr && n_rec > 0 && sizeof(IdT) >= 2;
+            f.seq_len = 0; f.pad_side = 0;
+            if (fuse) {
+                f.seq_len = h->cfg.seq_len; f.pad_side = h->cfg.pad_side;
+                f.e.ids = d_batch; f.e.ids_cap = n_rec * (int64_t)h->cfg.seq_len;
+            }
             const int64_t nthr = std::max<int64_t>(n_rec, n_wtiles);
             fa::fasta_parse_kernel<<<(unsigned)std::max<int64_t>(1, (nthr + 255) / 256), 256, 0, st>>>(f);
             launch_pdl1(fa::offsets_scan_kernel, (int)nb_scan, fa::OS_NT, 0, st, true, (const int32_t *)c.fa_tok, n_rec, out_off, (int64_t)0, c.descs, a.gen, c.d_status);
             int fgrid = (int)std::min<int64_t>((n_wtiles + fa::FW_WARPS - 1) / fa::FW_WARPS, (int64_t)h->sm_count * h->fasta_ctas_per_sm);
             fgrid = std::max(fgrid, 1);
             if (h->grid_cap > 0) fgrid = std::min(fgrid, h->grid_cap);
-            launch_fasta<IdT>(f, kk, fgrid, st);
+            if (fuse) {
+                fa::PadFillArgs pf;
+                pf.out_off = out_off; pf.n_rows = n_rec; pf.batch_ids = d_batch; pf.mask = d_mask;
+                pf.seq_len = h->cfg.seq_len; pf.pad_side = h->cfg.pad_side; pf.pad_id = h->cfg.pad_id;
+                int pgrid = (int)std::min<int64_t>(n_rec, (int64_t)h->sm_count * 16);
+                if (h->grid_cap > 0) pgrid = std::min(pgrid, h->grid_cap);
+                launch_pdl1(fa::pad_fill_kernel, pgrid, 256, 0, st, true, pf);
+                launch_fasta<int32_t>(f, kk, fgrid, st);                 // the batch holds int32 whatever the id type
+                h->launches += 1;
+            } else launch_fasta<IdT>(f, kk, fgrid, st);
             CU(cudaGetLastError());
             h->launches += 3;
             rc = ctx_next_gen(h, c, st); if (rc) return rc;      // the scan above used this generation's chain words
             a.gen = c.gen; a.run_if = c.fa_flag;
             chained = true;
+            f_fused = fuse;
             c.fa_tried = true;
         }
         // an input that gives every CTA at most one tile is encoded in ONE launch: the record range of a tile is searched
@@ -373,6 +397,12 @@ int launch_tiles(dnatok_t *h, EncCtx &c, const EncParams &prm, const uint8_t *d_
             h->launches += 1;
         }
         launch_strip<IdT>(a, kk, grid, st, chained);
+        if (chained && f_fused) {
+            // the chained-scan encoder's ids go through the pad kernel, which like it returns at once unless the flag is set
+            CU(cudaGetLastError());
+            rc = pad_on(h, ids, out_off, n_rec, d_batch, d_mask, st, ids_cap, c.fa_flag); if (rc) return rc;
+            *fused = true;
+        }
     }
     CU(cudaGetLastError());
     c.ticket_base += (unsigned long long)n_tiles + (unsigned long long)grid;
@@ -405,12 +435,15 @@ int ctx_reserve_bpe(dnatok_t *h, EncCtx &c, int64_t n_bytes, int64_t n_rec, cuda
 
 
 int encode_on(dnatok_t *h, EncCtx &c, const uint8_t *d_bytes, int64_t n_bytes, const int64_t *d_rec_off,
-              int64_t n_rec, int64_t off_bias, void *d_ids, int64_t ids_cap, int64_t *d_out_off, cudaStream_t st) {
+              int64_t n_rec, int64_t off_bias, void *d_ids, int64_t ids_cap, int64_t *d_out_off, cudaStream_t st,
+              int32_t *d_batch = nullptr, uint8_t *d_mask = nullptr, bool *fused = nullptr) {
     const dnatok_config &cfg = h->cfg;
     if (cfg.mode != DNATOK_BPE) {
         if (cfg.id_dtype == DNATOK_I16)
-            return launch_tiles<int16_t>(h, c, h->prm, d_bytes, n_bytes, d_rec_off, n_rec, off_bias, d_ids, ids_cap, d_out_off, st);
-        return launch_tiles<int32_t>(h, c, h->prm, d_bytes, n_bytes, d_rec_off, n_rec, off_bias, d_ids, ids_cap, d_out_off, st);
+            return launch_tiles<int16_t>(h, c, h->prm, d_bytes, n_bytes, d_rec_off, n_rec, off_bias, d_ids, ids_cap, d_out_off, st,
+                                         d_batch, d_mask, fused);
+        return launch_tiles<int32_t>(h, c, h->prm, d_bytes, n_bytes, d_rec_off, n_rec, off_bias, d_ids, ids_cap, d_out_off, st,
+                                     d_batch, d_mask, fused);
     }
     // BPE: pass A = compact kept classes + kept-base CSR offsets (the single-nt encoder with class ids),
     //      pass B = merge kernel per read, pass C = offsets scan, pass D = gather into ids_out
@@ -478,9 +511,10 @@ int encode_on(dnatok_t *h, EncCtx &c, const uint8_t *d_bytes, int64_t n_bytes, c
 }
 
 int pad_on(dnatok_t *h, const void *d_ids, const int64_t *d_out_off, int64_t n_rec, int32_t *d_batch,
-           uint8_t *d_mask, cudaStream_t st, int64_t ids_cap = INT64_MAX) {
+           uint8_t *d_mask, cudaStream_t st, int64_t ids_cap = INT64_MAX, const uint32_t *run_if = nullptr) {
     if (n_rec == 0) return DNATOK_OK;
     PadArgs a;
+    a.run_if = run_if;
     a.ids = d_ids; a.out_off = d_out_off; a.n_rows = n_rec; a.batch_ids = d_batch; a.mask = d_mask;
     a.seq_len = h->cfg.seq_len; a.pad_side = h->cfg.pad_side; a.pad_id = h->cfg.pad_id;
     a.ids_cap = ids_cap;
@@ -797,6 +831,22 @@ int dnatok_encode(dnatok_t *h, const uint8_t *d_bytes, int64_t n_bytes, const in
                      d_out_offsets, (cudaStream_t)stream);
 }
 
+int dnatok_encode_pad(dnatok_t *h, const uint8_t *d_bytes, int64_t n_bytes, const int64_t *d_rec_offsets,
+                      int64_t n_records, void *d_ids_out, int64_t ids_capacity, int64_t *d_out_offsets,
+                      int32_t *d_batch_ids, uint8_t *d_mask, void *stream) {
+    if (!h) return DNATOK_EINVAL;
+    if (h->cfg.seq_len <= 0) return fail(h, DNATOK_EINVAL, "dnatok_encode_pad: handle was created with seq_len == 0");
+    if (n_bytes < 0 || n_records < 0 || ids_capacity < 0 || !d_rec_offsets || !d_out_offsets ||
+        (n_bytes > 0 && !d_bytes) || (ids_capacity > 0 && !d_ids_out) || (n_records > 0 && !d_batch_ids))
+        return fail(h, DNATOK_EINVAL, "dnatok_encode_pad: bad argument");
+    USE_DEVICE(h);
+    bool fused = false;
+    int rc = encode_on(h, h->ctx, d_bytes, n_bytes, d_rec_offsets, n_records, 0, d_ids_out, ids_capacity, d_out_offsets,
+                       (cudaStream_t)stream, d_batch_ids, d_mask, &fused);
+    if (rc || fused) return rc;
+    return pad_on(h, d_ids_out, d_out_offsets, n_records, d_batch_ids, d_mask, (cudaStream_t)stream, ids_capacity);
+}
+
 int dnatok_pad(dnatok_t *h, const void *d_ids, const int64_t *d_out_offsets, int64_t n_records,
                int32_t *d_batch_ids, uint8_t *d_mask, void *stream) {
     if (!h) return DNATOK_EINVAL;
@@ -871,6 +921,8 @@ static int stream_run(dnatok_t *h, const uint8_t *h_pinned, dnatok_fill_fn fill,
         CU(cudaEventRecord(S.ev_off, st));
         // encode the whole records [ra, rb): buffer starts at host offset data0
         const int64_t nb = std::max<int64_t>(0, (rows > 0 ? h_rec_offsets[rb] : data0) - data0);
+        // (encode, then pad: a batch hands out its CSR ids as well as its rows, so the fused call of dnatok_encode_pad, which
+        // leaves the ids unwritten, is not used here -- and a chunk's kernels are a tenth of its host-to-device copy anyway)
         rc = encode_on(h, S.ctx, d_chunk - carry, nb, S.d_recoff, rows, data0, S.d_ids, R.carry_cap + C,
                        S.d_out_off, st);
         if (rc) return rc;

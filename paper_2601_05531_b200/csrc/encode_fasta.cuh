@@ -50,6 +50,10 @@ struct FastaArgs {
     int32_t *wt_first;           // [n_wtiles] record that holds the tile's first byte (first record starting behind it if none)
     uint32_t *irregular;         // set when the input does not have the regular layout
     int32_t n_wtiles;
+    // seq_len > 0: the tokens go straight into the padded batch (e.ids = batch_ids[n_rec][seq_len] int32, e.ids_cap = n_rec * seq_len):
+    // token j < seq_len of record r at column j + (pad_side == 0 ? seq_len - min(tokens, seq_len) : 0) -- pad_kernel.cuh's rule; the
+    // pad columns and the mask are pad_fill_kernel's
+    int32_t seq_len, pad_side;
 };
 
 struct SmemFa {
@@ -216,6 +220,48 @@ __global__ void __launch_bounds__(OS_NT) offsets_scan_kernel(const int32_t *tok,
     long long ex = s_base + woff + inc - run + out_bias;
 #pragma unroll
     for (int i = 0; i < OS_PER; ++i) { if (r0 + i < n_rec) out_off[r0 + i] = ex; ex += v[i]; }
+}
+
+// ---- the columns of the padded batch that hold no token, and the whole mask, from the token counts alone (fused path: the
+// encoder behind writes the tokens into their columns itself).  One CTA per row, four columns per thread and step. ----
+struct PadFillArgs {
+    const int64_t *out_off; int64_t n_rows;
+    int32_t *batch_ids; uint8_t *mask;          // mask may be null
+    int32_t seq_len, pad_side, pad_id;
+};
+__global__ void __launch_bounds__(256) pad_fill_kernel(const __grid_constant__ PadFillArgs A) {
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+    asm volatile("griddepcontrol.wait;" ::: "memory");           // out_offsets come from the scan in front
+    const int L = A.seq_len;
+    const bool vec = (L & 3) == 0 && (reinterpret_cast<uintptr_t>(A.batch_ids) & 15) == 0 &&
+                     (A.mask == nullptr || (reinterpret_cast<uintptr_t>(A.mask) & 3) == 0);
+    for (int64_t r = blockIdx.x; r < A.n_rows; r += gridDim.x) {
+        const int64_t tok = A.out_off[r + 1] - A.out_off[r];
+        const int m = (int)(tok < L ? tok : L);
+        const int col0 = A.pad_side == 0 ? L - m : 0;            // the kept tokens sit in columns [col0, col0 + m)
+        int32_t *row = A.batch_ids + r * L;
+        uint8_t *mrow = A.mask ? A.mask + r * L : nullptr;
+        if (vec) {
+            for (int c = threadIdx.x * 4; c < L; c += blockDim.x * 4) {
+                uint32_t mk = 0;
+                int n_in = 0;
+#pragma unroll
+                for (int j = 0; j < 4; ++j) { const bool in = c + j >= col0 && c + j < col0 + m; mk |= (uint32_t)in << (8 * j); n_in += in; }
+                if (n_in == 0) *reinterpret_cast<int4 *>(row + c) = make_int4(A.pad_id, A.pad_id, A.pad_id, A.pad_id);
+                else if (n_in < 4) {
+#pragma unroll
+                    for (int j = 0; j < 4; ++j) if (!((mk >> (8 * j)) & 1u)) row[c + j] = A.pad_id;
+                }
+                if (mrow) *reinterpret_cast<uint32_t *>(mrow + c) = mk;
+            }
+        } else {
+            for (int c = threadIdx.x; c < L; c += blockDim.x) {
+                const bool in = c >= col0 && c < col0 + m;
+                if (!in) row[c] = A.pad_id;
+                if (mrow) mrow[c] = in ? 1 : 0;
+            }
+        }
+    }
 }
 
 // ---- emission from a warp's private stream (code words cw, flag words fw; base u at bits 31-2(u&15).. of cw[u>>4]) ----
@@ -421,6 +467,14 @@ __global__ void __launch_bounds__(FW_WARPS * 32, 3) encode_fasta_kernel(const __
                 nwin = n_r / (uint32_t)k;
             }
             const int64_t T_r = __ldcg(A.out_off + r);
+            // destination index of the record's token 0, and the number of its tokens that have a place at all
+            int64_t g_base = T_r;
+            uint32_t jcap = 0xffffffffu;
+            if (F.seq_len > 0) {
+                const int64_t Ttok = __ldcg(A.out_off + r + 1) - T_r, L = F.seq_len;
+                g_base = r * L + (F.pad_side == 0 ? L - (Ttok < L ? Ttok : L) : 0);
+                jcap = (uint32_t)L;
+            }
             // the warp's stream starts empty (edge words are OR-ed in)
             for (int i = lane; i < FW_WORDS / 4; i += 32) reinterpret_cast<uint4 *>(cw)[i] = make_uint4(0, 0, 0, 0);
             __syncwarp();
@@ -741,7 +795,8 @@ __global__ void __launch_bounds__(FW_WARPS * 32, 3) encode_fasta_kernel(const __
             const int ufirst = (int)(jfirst * (uint32_t)k - K0);                 //   and the stream position of its first base
             int nwp = ufirst < nK ? (int)((uint32_t)(nK - ufirst + k - 1) / (uint32_t)k) : 0;   // windows that start in the piece
             if (nwin != FAR && jfirst + (uint32_t)nwp > nwin) nwp = nwin > jfirst ? (int)(nwin - jfirst) : 0;
-            const int64_t g0 = T_r + jfirst;                                     // global token index of the first of them
+            if (jfirst + (uint32_t)nwp > jcap) nwp = jcap > jfirst ? (int)(jcap - jfirst) : 0;
+            const int64_t g0 = g_base + jfirst;                                  // destination index of the first of them
             IdT *const idp = ids + g0;
             int xa = nwp, xb = nwp;                                              // windows [xa, xb) go through the 16-byte group cutter
             if (vec_ok) {
@@ -768,10 +823,10 @@ __global__ void __launch_bounds__(FW_WARPS * 32, 3) encode_fasta_kernel(const __
                     for (int64_t bb = b0 + lane; bb < b1; bb += 32) {
                         const uint32_t c = w_class(cw, fw, (int)(bb - K0));
                         const int32_t id = c <= CLS_N ? (P.remap4 ? P.nt_ids[c] : (int32_t)(P.base_id + P.four_k + c)) : P.unk_id;
-                        store_id<IdT>(A, T_r + nwin + (bb - tb0), id);
+                        if (nwin + (uint32_t)(bb - tb0) < jcap) store_id<IdT>(A, g_base + nwin + (bb - tb0), id);
                     }
                 } else if (P.tail_policy == TAIL_UNK) {
-                    if (lane == 0 && n_r > tb0 && tb0 >= K0 && tb0 < K0 + nK) store_id<IdT>(A, T_r + nwin, P.unk_id);
+                    if (lane == 0 && n_r > tb0 && tb0 >= K0 && tb0 < K0 + nK && nwin < jcap) store_id<IdT>(A, g_base + nwin, P.unk_id);
                 }
             }
             __syncwarp();

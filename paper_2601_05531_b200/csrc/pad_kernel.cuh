@@ -18,11 +18,13 @@ struct PadArgs {
     uint8_t *mask;              // may be null
     int32_t seq_len, pad_side, pad_id;
     int64_t ids_cap;            // ids beyond it were never written (an encode that overflowed): read as pad_id
+    const uint32_t *run_if;     // non-null: the kernel returns at once unless *run_if != 0 (the fused path's fall-back)
 };
 
 // one CTA per row (grid-stride), each thread writes 4 consecutive columns per step
 template <typename IdT>
 __global__ void __launch_bounds__(256) pad_rows_kernel(const __grid_constant__ PadArgs A) {
+    if (A.run_if && *A.run_if == 0u) return;
     const IdT *ids = reinterpret_cast<const IdT *>(A.ids);
     const int L = A.seq_len;
     // 16-byte id stores and 4-byte mask stores need aligned rows: seq_len a multiple of 4 and aligned base pointers

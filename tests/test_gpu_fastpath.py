@@ -304,3 +304,89 @@ def test_threshold_small_inputs_skip_the_fast_path_by_default():
     run(data, offs, True, mode="kmer", k=6)                                    # 4 MiB and more: regular-layout encoder
     dn.FAST_PATH = 0
     run(data, offs, False, mode="kmer", k=6)
+
+
+# ------------------------------------------------------------------------------------------------ fused encode + pad
+def run_padded(data, offsets, taken, seq_len, pad_side, misalign=0, **kw):
+    """dnatok_encode_pad against oracle encode + pad; a call served by the regular-layout encoder must leave ids_out untouched"""
+    if not isinstance(data, np.ndarray):
+        data = np.frombuffer(bytes(data), dtype=np.uint8)
+    offsets = np.asarray(offsets, dtype=np.int64)
+    okw = dict(kw)
+    okw["mode"] = {"single_nt": oracle.SINGLE_NT, "kmer": oracle.KMER, "bpe": oracle.BPE}[okw.get("mode", "kmer")]
+    okw.pop("id_dtype", None)
+    okw.pop("max_record_bytes", None)
+    ocfg = oracle.Config(seq_len=seq_len, pad_side=pad_side, **okw)
+    want_ids, want_off = oracle.encode(data, offsets, ocfg)
+    want_b, want_m = oracle.pad(want_ids, want_off, ocfg)
+    tok = dn.DNATok(seq_len=seq_len, pad_side=pad_side, **kw)
+    buf = torch.zeros(data.size + misalign + 64, dtype=torch.uint8, device="cuda")
+    d = buf[misalign:misalign + data.size]
+    d.copy_(torch.from_numpy(np.ascontiguousarray(data)))
+    o = torch.from_numpy(offsets).cuda()
+    poison = -12345 if tok.id_torch_dtype == torch.int32 else -1234
+    ids = torch.full((max(data.size, 1),), poison, dtype=tok.id_torch_dtype, device="cuda")
+    n_rec = offsets.size - 1
+    batch = torch.full((n_rec, seq_len), -777, dtype=torch.int32, device="cuda")
+    mask = torch.full((n_rec, seq_len), 9, dtype=torch.uint8, device="cuda")
+    b, m, out = tok.encode_padded(d, o, ids_out=ids, batch_ids=batch, mask=mask)
+    tok.check()
+    got_taken = tok.fast_path_taken()
+    assert np.array_equal(out.cpu().numpy(), want_off)
+    gb, gm = b.cpu().numpy(), m.cpu().numpy()
+    assert np.array_equal(gm, want_m), np.argwhere(gm != want_m)[:5]
+    bad = np.argwhere(gb != want_b)
+    assert bad.size == 0, (bad[:5], gb[tuple(bad[0])], want_b[tuple(bad[0])])
+    if taken is not None:
+        assert got_taken == taken
+    if got_taken:
+        assert bool((ids == poison).all()), "the CSR ids were written although the tokens went straight into the batch"
+    return got_taken
+
+
+@pytest.mark.parametrize("pad_side", [0, 1])
+@pytest.mark.parametrize("seq_len", [512, 333, 8, 2048])
+def test_fused_pad_on_wrapped_records(seq_len, pad_side):
+    rng = random.Random(seq_len + pad_side)
+    # records from empty to several times seq_len tokens (truncation: the first seq_len tokens are kept)
+    data, offs = fasta(rng, 14, 60, 0, 9000, alphabet="ACGTACGTACGTN")
+    for kw in (dict(mode="kmer", k=6), dict(mode="kmer", k=6, id_dtype=2), dict(mode="single_nt"), dict(mode="kmer", k=3, tail_policy=2),
+               dict(mode="kmer", k=5, tail_policy=1), dict(mode="kmer", k=15)):
+        run_padded(data, offs, True, seq_len, pad_side, **kw)
+    run_padded(data, offs, True, seq_len, pad_side, misalign=5, mode="kmer", k=4)
+
+
+def test_fused_pad_one_line_records_config5_shape():
+    rng = random.Random(21)
+    recs = [("".join(rng.choice("ACGT") for _ in range(rng.choice([4096, 4096, 100, 5000, 0, 1]))) + "\n").encode() for _ in range(40)]
+    offs = np.cumsum([0] + [len(r) for r in recs])
+    run_padded(b"".join(recs), offs, True, 683, 0, mode="kmer", k=6)          # 4096 / 6 = 682.67: full rows, short rows, cut rows
+    run_padded(b"".join(recs), offs, True, 683, 1, mode="kmer", k=6)
+    run_padded(b"".join(recs), offs, True, 700, 0, mode="kmer", k=6, tail_policy=2)
+
+
+def test_fused_pad_falls_back_on_irregular_input_and_small_inputs_skip_it():
+    rng = random.Random(22)
+    data, offs = fasta(rng, 10, 60, 100, 6000)
+    bad = data.copy()
+    p = int(offs[4]) + 700
+    p += int(bad[p] == 10)
+    bad[p] = 10                                                                # a line cut in two: the chained-scan encoder + pad kernel
+    run_padded(bad, offs, False, 256, 0, mode="kmer", k=6)
+    run_padded(bad, offs, False, 256, 1, mode="kmer", k=6, id_dtype=2)
+    dn.FAST_PATH = 1
+    run_padded(data, offs, False, 256, 0, mode="kmer", k=6)                    # under the size threshold: encode + pad as before
+    dn.FAST_PATH = 0
+    run_padded(data, offs, False, 256, 0, mode="kmer", k=6)
+
+
+def test_fused_entry_point_serves_bpe_and_dense_specs_through_the_pad_kernel():
+    import dnagen
+    rng = random.Random(23)
+    merges = dnagen.merge_table(seed=3, n_merges=200, corpus_bases=8192)
+    recs = ["".join(rng.choice("ACGTN") for _ in range(rng.randrange(0, 400))).encode() for _ in range(30)]
+    offs = np.cumsum([0] + [len(r) for r in recs])
+    run_padded(b"".join(recs), offs, False, 64, 0, mode="bpe", merges=merges)
+    lut = oracle.default_lut().copy()
+    lut[lut == oracle.CLS_SKIP] = oracle.CLS_UNK                               # no SKIP class + no header strip: the dense encoder
+    run_padded(b"".join(recs), offs, False, 64, 1, mode="kmer", k=3, class_lut=lut, strip_headers=False)

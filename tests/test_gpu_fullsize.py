@@ -162,7 +162,7 @@ def test_capped_grid_pad(grid_cap):
     w = dnagen.config3(total_bases=300_000, lo=1000, hi=9000)
     tok = dn.DNATok(mode="kmer", k=6, seq_len=700)
     d, o = torch.from_numpy(w.data).cuda(), torch.from_numpy(w.offsets).cuda()
-    batch, mask = tok.encode_padded(d, o)
+    batch, mask, _ = tok.encode_padded(d, o)
     tok.check()
     cfg = oracle.Config(mode=oracle.KMER, k=6, seq_len=700)
     want_ids, want_off = oracle.encode(w.data, w.offsets, cfg)

@@ -386,7 +386,7 @@ def test_pad_handworked(golden_dir):
     data = np.frombuffer((g["record0"] + g["record1"]).encode(), dtype=np.uint8).copy()
     for side, key in ((0, "kmer3_pad5_left"), (1, "kmer3_pad5_right")):
         tok = dn.DNATok(mode="kmer", k=3, seq_len=5, pad_side=side)
-        batch, mask = tok.encode_padded(torch.from_numpy(data).cuda(), torch.tensor(g["rec_offsets"]).cuda())
+        batch, mask, _ = tok.encode_padded(torch.from_numpy(data).cuda(), torch.tensor(g["rec_offsets"]).cuda())
         tok.check()
         assert batch.cpu().tolist() == g[key]["ids"] and mask.cpu().tolist() == g[key]["mask"]
 
