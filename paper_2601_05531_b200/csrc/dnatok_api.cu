@@ -261,21 +261,21 @@ void launch_pdl1(K kernel, int grid, int block, size_t smem, cudaStream_t st, bo
     cfg.attrs = attr; cfg.numAttrs = pdl ? 1 : 0;
     cudaLaunchKernelEx(&cfg, kernel, args...);
 }
-template <typename IdT>
+template <typename IdT, bool FUSED = false>
 void launch_fasta(const fa::FastaArgs &f, int kk, int grid, cudaStream_t st) {
     using namespace dtk::fa;
     constexpr bool wide = sizeof(IdT) >= 2;
     const size_t sm = sizeof(SmemFa);
     switch (wide ? kk : 0) {
-        case 0: launch_pdl1(encode_fasta_kernel<IdT, 0>, grid, FW_WARPS * 32, sm, st, true, f); break;
-        case 1: launch_pdl1(encode_fasta_kernel<IdT, wide ? 1 : 0>, grid, FW_WARPS * 32, sm, st, true, f); break;
-        case 2: launch_pdl1(encode_fasta_kernel<IdT, wide ? 2 : 0>, grid, FW_WARPS * 32, sm, st, true, f); break;
-        case 3: launch_pdl1(encode_fasta_kernel<IdT, wide ? 3 : 0>, grid, FW_WARPS * 32, sm, st, true, f); break;
-        case 4: launch_pdl1(encode_fasta_kernel<IdT, wide ? 4 : 0>, grid, FW_WARPS * 32, sm, st, true, f); break;
-        case 5: launch_pdl1(encode_fasta_kernel<IdT, wide ? 5 : 0>, grid, FW_WARPS * 32, sm, st, true, f); break;
-        case 6: launch_pdl1(encode_fasta_kernel<IdT, wide ? 6 : 0>, grid, FW_WARPS * 32, sm, st, true, f); break;
-        case 8: launch_pdl1(encode_fasta_kernel<IdT, wide ? 8 : 0>, grid, FW_WARPS * 32, sm, st, true, f); break;
-        default: launch_pdl1(encode_fasta_kernel<IdT, wide ? -1 : 0>, grid, FW_WARPS * 32, sm, st, true, f); break;
+        case 0: launch_pdl1(encode_fasta_kernel<IdT, 0, FUSED>, grid, FW_WARPS * 32, sm, st, true, f); break;
+        case 1: launch_pdl1(encode_fasta_kernel<IdT, wide ? 1 : 0, FUSED>, grid, FW_WARPS * 32, sm, st, true, f); break;
+        case 2: launch_pdl1(encode_fasta_kernel<IdT, wide ? 2 : 0, FUSED>, grid, FW_WARPS * 32, sm, st, true, f); break;
+        case 3: launch_pdl1(encode_fasta_kernel<IdT, wide ? 3 : 0, FUSED>, grid, FW_WARPS * 32, sm, st, true, f); break;
+        case 4: launch_pdl1(encode_fasta_kernel<IdT, wide ? 4 : 0, FUSED>, grid, FW_WARPS * 32, sm, st, true, f); break;
+        case 5: launch_pdl1(encode_fasta_kernel<IdT, wide ? 5 : 0, FUSED>, grid, FW_WARPS * 32, sm, st, true, f); break;
+        case 6: launch_pdl1(encode_fasta_kernel<IdT, wide ? 6 : 0, FUSED>, grid, FW_WARPS * 32, sm, st, true, f); break;
+        case 8: launch_pdl1(encode_fasta_kernel<IdT, wide ? 8 : 0, FUSED>, grid, FW_WARPS * 32, sm, st, true, f); break;
+        default: launch_pdl1(encode_fasta_kernel<IdT, wide ? -1 : 0, FUSED>, grid, FW_WARPS * 32, sm, st, true, f); break;
     }
 }
 template <typename IdT>
@@ -377,7 +377,7 @@ int launch_tiles(dnatok_t *h, EncCtx &c, const EncParams &prm, const uint8_t *d_
                 int pgrid = (int)std::min<int64_t>(n_rec, (int64_t)h->sm_count * 16);
                 if (h->grid_cap > 0) pgrid = std::min(pgrid, h->grid_cap);
                 launch_pdl1(fa::pad_fill_kernel, pgrid, 256, 0, st, true, pf);
-                launch_fasta<int32_t>(f, kk, fgrid, st);                 // the batch holds int32 whatever the id type
+                launch_fasta<int32_t, true>(f, kk, fgrid, st);           // the batch holds int32 whatever the id type
                 h->launches += 1;
             } else launch_fasta<IdT>(f, kk, fgrid, st);
             CU(cudaGetLastError());
@@ -789,7 +789,12 @@ int dnatok_create(const dnatok_config *cfg_in, int device, dnatok_t **out) {
 #define DTK_FA(T) (const void *)fa::encode_fasta_kernel<T, 0>, (const void *)fa::encode_fasta_kernel<T, 1>, (const void *)fa::encode_fasta_kernel<T, 2>, \
                   (const void *)fa::encode_fasta_kernel<T, 3>, (const void *)fa::encode_fasta_kernel<T, 4>, (const void *)fa::encode_fasta_kernel<T, 5>, \
                   (const void *)fa::encode_fasta_kernel<T, 6>, (const void *)fa::encode_fasta_kernel<T, 8>, (const void *)fa::encode_fasta_kernel<T, -1>
-        const void *kfa[] = {DTK_FA(int32_t), DTK_FA(int16_t), (const void *)fa::encode_fasta_kernel<uint8_t, 0>};
+#define DTK_FAF (const void *)fa::encode_fasta_kernel<int32_t, 0, true>, (const void *)fa::encode_fasta_kernel<int32_t, 1, true>, \
+                (const void *)fa::encode_fasta_kernel<int32_t, 2, true>, (const void *)fa::encode_fasta_kernel<int32_t, 3, true>, \
+                (const void *)fa::encode_fasta_kernel<int32_t, 4, true>, (const void *)fa::encode_fasta_kernel<int32_t, 5, true>, \
+                (const void *)fa::encode_fasta_kernel<int32_t, 6, true>, (const void *)fa::encode_fasta_kernel<int32_t, 8, true>, \
+                (const void *)fa::encode_fasta_kernel<int32_t, -1, true>
+        const void *kfa[] = {DTK_FA(int32_t), DTK_FA(int16_t), DTK_FAF, (const void *)fa::encode_fasta_kernel<uint8_t, 0>};
 #undef DTK_FA
         for (const void *kf : kfa)
             if (cudaFuncSetAttribute(kf, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(fa::SmemFa)) != cudaSuccess)

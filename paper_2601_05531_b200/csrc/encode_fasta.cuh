@@ -385,7 +385,8 @@ __device__ __forceinline__ int clamp64(int64_t v) { return v < 0 ? 0 : (v > 64 ?
 
 // ======================================================================================================
 // KK: the emission variant compiled in -- 0 single-nt, 1..6 / 8 that k, -1 every variant behind a run-time switch
-template <typename IdT, int KK>
+// FUSED: the tokens go into the padded batch (FastaArgs::seq_len > 0; IdT = int32_t)
+template <typename IdT, int KK, bool FUSED = false>
 __global__ void __launch_bounds__(FW_WARPS * 32, 3) encode_fasta_kernel(const __grid_constant__ FastaArgs F) {
     extern __shared__ __align__(16) uint8_t smem_raw[];
     SmemFa &sm = *reinterpret_cast<SmemFa *>(smem_raw);
@@ -470,7 +471,7 @@ __global__ void __launch_bounds__(FW_WARPS * 32, 3) encode_fasta_kernel(const __
             // destination index of the record's token 0, and the number of its tokens that have a place at all
             int64_t g_base = T_r;
             uint32_t jcap = 0xffffffffu;
-            if (F.seq_len > 0) {
+            if (FUSED) {
                 const int64_t Ttok = __ldcg(A.out_off + r + 1) - T_r, L = F.seq_len;
                 g_base = r * L + (F.pad_side == 0 ? L - (Ttok < L ? Ttok : L) : 0);
                 jcap = (uint32_t)L;
@@ -795,7 +796,7 @@ __global__ void __launch_bounds__(FW_WARPS * 32, 3) encode_fasta_kernel(const __
             const int ufirst = (int)(jfirst * (uint32_t)k - K0);                 //   and the stream position of its first base
             int nwp = ufirst < nK ? (int)((uint32_t)(nK - ufirst + k - 1) / (uint32_t)k) : 0;   // windows that start in the piece
             if (nwin != FAR && jfirst + (uint32_t)nwp > nwin) nwp = nwin > jfirst ? (int)(nwin - jfirst) : 0;
-            if (jfirst + (uint32_t)nwp > jcap) nwp = jcap > jfirst ? (int)(jcap - jfirst) : 0;
+            if (FUSED && jfirst + (uint32_t)nwp > jcap) nwp = jcap > jfirst ? (int)(jcap - jfirst) : 0;
             const int64_t g0 = g_base + jfirst;                                  // destination index of the first of them
             IdT *const idp = ids + g0;
             int xa = nwp, xb = nwp;                                              // windows [xa, xb) go through the 16-byte group cutter
@@ -823,10 +824,10 @@ __global__ void __launch_bounds__(FW_WARPS * 32, 3) encode_fasta_kernel(const __
                     for (int64_t bb = b0 + lane; bb < b1; bb += 32) {
                         const uint32_t c = w_class(cw, fw, (int)(bb - K0));
                         const int32_t id = c <= CLS_N ? (P.remap4 ? P.nt_ids[c] : (int32_t)(P.base_id + P.four_k + c)) : P.unk_id;
-                        if (nwin + (uint32_t)(bb - tb0) < jcap) store_id<IdT>(A, g_base + nwin + (bb - tb0), id);
+                        if (!FUSED || nwin + (uint32_t)(bb - tb0) < jcap) store_id<IdT>(A, g_base + nwin + (bb - tb0), id);
                     }
                 } else if (P.tail_policy == TAIL_UNK) {
-                    if (lane == 0 && n_r > tb0 && tb0 >= K0 && tb0 < K0 + nK && nwin < jcap) store_id<IdT>(A, g_base + nwin, P.unk_id);
+                    if (lane == 0 && n_r > tb0 && tb0 >= K0 && tb0 < K0 + nK && (!FUSED || nwin < jcap)) store_id<IdT>(A, g_base + nwin, P.unk_id);
                 }
             }
             __syncwarp();
