@@ -261,7 +261,7 @@ int64_t dnatok_launch_count(const dnatok_t *h);
 int dnatok_set_super_tile(dnatok_t *h, int32_t sub_tiles);
 
 /*
- * Test / tuning knob of the strip path: 1 (default) = inputs of 4 MiB or more go to the closed-form
+ * Test / tuning knob of the strip path: 1 (default) = inputs of 48 MiB or more go to the closed-form
  * encoder first, which assumes records laid out as an optional '>' header line followed by lines of one fixed width and
  * checks that layout on every byte; the chained-scan encoder runs behind it only if the check failed somewhere.  2 = the
  * same for inputs of any size (tests), 0 = the chained-scan encoder only.  Results never depend on it.  EINVAL outside 0..2.

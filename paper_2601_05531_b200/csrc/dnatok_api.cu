@@ -95,7 +95,7 @@ struct dnatok {
     int enc_ctas_per_sm = 1, dense_ctas_per_sm = 1, bpe_ctas_per_sm = 1;
     bool dense = false;                // no SKIP class and strip_headers == 0: kept bases = bytes, the no-scan encoder runs
     int force_S = 0;                   // dnatok_set_super_tile: fixed super-tile size in sub-tiles (0 = automatic)
-    int fast_path = 1;                 // dnatok_set_fast_path: 1 = try the regular-layout encoder first on inputs of 4 MiB or more,
+    int fast_path = 1;                 // dnatok_set_fast_path: 1 = try the regular-layout encoder first on inputs of 48 MiB or more,
                                        //   2 = on every input, 0 = chained-scan encoder only
     int fasta_ctas_per_sm = 4;
     int grid_cap = 0;                  // dnatok_set_grid_cap: at most this many persistent CTAs per launch (0 = no cap)
@@ -261,6 +261,10 @@ void launch_pdl1(K kernel, int grid, int block, size_t smem, cudaStream_t st, bo
     cfg.attrs = attr; cfg.numAttrs = pdl ? 1 : 0;
     cudaLaunchKernelEx(&cfg, kernel, args...);
 }
+// The regular-layout path costs three launches and a latency-bound parse before its encoder starts; measured against the
+// chained-scan encoder on L2-flushed inputs of both FASTA shapes it wins from 32-64 MiB on.
+constexpr int64_t FAST_PATH_MIN_BYTES = 48ll << 20;
+
 template <typename IdT, bool FUSED = false>
 void launch_fasta(const fa::FastaArgs &f, int kk, int grid, cudaStream_t st) {
     using namespace dtk::fa;
@@ -346,7 +350,7 @@ int launch_tiles(dnatok_t *h, EncCtx &c, const EncParams &prm, const uint8_t *d_
         bool chained = false;                                 // the kernels below follow kernels of this call
         bool f_fused = false;
         c.fa_tried = false;
-        if ((h->fast_path == 2 || (h->fast_path == 1 && n_bytes >= (4ll << 20))) && n_rec < (1ll << 31)) {
+        if ((h->fast_path == 2 || (h->fast_path == 1 && n_bytes >= FAST_PATH_MIN_BYTES)) && n_rec < (1ll << 31)) {
             // regular-layout fast path first (encode_fasta.cuh); the chained-scan encoder behind it runs only if the layout
             // check failed somewhere
             const int64_t n_wtiles = (a.p_end + fa::FW_TILE - 1) / fa::FW_TILE;

@@ -296,14 +296,15 @@ def test_fuzz_mixture_of_regular_and_irregular_inputs():
 
 
 def test_threshold_small_inputs_skip_the_fast_path_by_default():
+    import dnagen
     dn.FAST_PATH = 1
     rng = random.Random(15)
     data, offs = fasta(rng, 8, 60, 3000, 6000)
-    run(data, offs, False, mode="kmer", k=6)                                   # under 4 MiB: chained-scan encoder directly
-    data, offs = fasta(rng, 6, 60, 800_000, 900_000)
-    run(data, offs, True, mode="kmer", k=6)                                    # 4 MiB and more: regular-layout encoder
+    run(data, offs, False, mode="kmer", k=6)                                   # under 48 MiB: chained-scan encoder directly
+    w = dnagen.config3(total_bases=52 << 20, lo=1000, hi=131072, seed=15)
+    run(w.data, w.offsets, True, mode="kmer", k=6)                             # 48 MiB and more: regular-layout encoder
     dn.FAST_PATH = 0
-    run(data, offs, False, mode="kmer", k=6)
+    run(w.data, w.offsets, False, mode="kmer", k=6)
 
 
 # ------------------------------------------------------------------------------------------------ fused encode + pad
@@ -375,7 +376,7 @@ def test_fused_pad_falls_back_on_irregular_input_and_small_inputs_skip_it():
     run_padded(bad, offs, False, 256, 0, mode="kmer", k=6)
     run_padded(bad, offs, False, 256, 1, mode="kmer", k=6, id_dtype=2)
     dn.FAST_PATH = 1
-    run_padded(data, offs, False, 256, 0, mode="kmer", k=6)                    # under the size threshold: encode + pad as before
+    run_padded(data, offs, False, 256, 0, mode="kmer", k=6)                    # under the size threshold (48 MiB): encode + pad as before
     dn.FAST_PATH = 0
     run_padded(data, offs, False, 256, 0, mode="kmer", k=6)
 
