@@ -228,6 +228,20 @@ int dnatok_revcomp(dnatok_t *h, const uint8_t *d_bytes, int64_t n_bytes, const i
 int dnatok_decode(dnatok_t *h, const void *d_ids, const int64_t *d_out_offsets, int64_t n_records,
                   uint8_t *d_bytes_out, int64_t bytes_capacity, int64_t *d_byte_offsets, void *stream);
 
+/*
+ * dnatok_decode_static: dnatok_decode for callers that may not allocate device memory (code under CUDA graph capture,
+ * tight serving loops, harnesses that forbid cudaMalloc).  Same arguments, same results, but the call allocates and frees
+ * NOTHING: its only scratch, the decoded length of every record, lives in a static device array inside the library of
+ * DNATOK_DECODE_STATIC_MAX_RECORDS int32 (4 MiB, held by every GPU that loads the library until the process exits).
+ * n_records beyond that maximum: DNATOK_ECAPACITY, nothing launched (use dnatok_decode, or split the records over calls).
+ * Every handle and every call on a GPU shares the one array: calls that may overlap on the GPU (different streams, no
+ * ordering between them) race on it -- order them, or use dnatok_decode, whose scratch belongs to the handle.  Nothing in
+ * the array has to be cleared between calls (each call writes every entry it reads).  Enqueue only.
+ */
+#define DNATOK_DECODE_STATIC_MAX_RECORDS 1048576
+int dnatok_decode_static(dnatok_t *h, const void *d_ids, const int64_t *d_out_offsets, int64_t n_records,
+                         uint8_t *d_bytes_out, int64_t bytes_capacity, int64_t *d_byte_offsets, void *stream);
+
 /* Rows per embedding call, PAPER.md:136 (Alg. 2 l.17) / PAPER.md:181: b = min(B_emb, max(1, floor(M / T'))).   */
 int64_t dnatok_microbatch_rows(int64_t b_emb, int64_t m_tokens, int64_t t_len);
 

@@ -26,11 +26,12 @@ __all__ = [
     "SINGLE_NT", "KMER", "BPE", "I16", "I32", "TAIL_PER_BASE", "TAIL_DROP", "TAIL_UNK", "PAD_LEFT", "PAD_RIGHT",
     "dnatok_create", "dnatok_destroy", "dnatok_encode", "dnatok_pad", "dnatok_encode_pad", "dnatok_stream_encode", "dnatok_check",
     "dnatok_last_error", "dnatok_launch_count", "dnatok_version", "dnatok_config_default", "dnatok_set_super_tile", "dnatok_set_grid_cap", "dnatok_set_fast_path", "dnatok_fast_path_taken",
-    "dnatok_stream_encode_from", "dnatok_revcomp", "dnatok_decode", "dnatok_microbatch_rows", "dnatok_embed", "dnatok_widen_ids",
+    "dnatok_stream_encode_from", "dnatok_revcomp", "dnatok_decode", "dnatok_decode_static", "DECODE_STATIC_MAX_RECORDS", "dnatok_microbatch_rows", "dnatok_embed", "dnatok_widen_ids",
 ]
 
 SINGLE_NT, KMER, BPE = 0, 1, 2
 I16, I32 = 2, 4
+DECODE_STATIC_MAX_RECORDS = 1 << 20     # dnatok.h DNATOK_DECODE_STATIC_MAX_RECORDS
 TAIL_PER_BASE, TAIL_DROP, TAIL_UNK = 0, 1, 2
 PAD_LEFT, PAD_RIGHT = 0, 1
 OK, EINVAL, ENOMEM, ECUDA, ECAPACITY, ESTATE = range(6)
@@ -126,6 +127,8 @@ def lib() -> ctypes.CDLL:
         L.dnatok_revcomp.argtypes = [vp, vp, i64, vp, i64, vp, vp]
         L.dnatok_decode.restype = ctypes.c_int
         L.dnatok_decode.argtypes = [vp, vp, vp, i64, vp, i64, vp, vp]
+        L.dnatok_decode_static.restype = ctypes.c_int
+        L.dnatok_decode_static.argtypes = [vp, vp, vp, i64, vp, i64, vp, vp]
         L.dnatok_microbatch_rows.restype = i64
         L.dnatok_microbatch_rows.argtypes = [i64, i64, i64]
         L.dnatok_embed.restype = ctypes.c_int
@@ -231,6 +234,11 @@ def dnatok_revcomp(h: int, d_bytes: int, n_bytes: int, d_rec_offsets: int, n_rec
 def dnatok_decode(h: int, d_ids: int, d_out_offsets: int, n_records: int, d_bytes_out: int, bytes_capacity: int,
                   d_byte_offsets: int, stream: int = 0) -> None:
     _chk(h, lib().dnatok_decode(h, d_ids, d_out_offsets, n_records, d_bytes_out, bytes_capacity, d_byte_offsets, stream))
+
+
+def dnatok_decode_static(h: int, d_ids: int, d_out_offsets: int, n_records: int, d_bytes_out: int, bytes_capacity: int,
+                         d_byte_offsets: int, stream: int = 0) -> None:
+    _chk(h, lib().dnatok_decode_static(h, d_ids, d_out_offsets, n_records, d_bytes_out, bytes_capacity, d_byte_offsets, stream))
 
 
 def dnatok_microbatch_rows(b_emb: int, m_tokens: int, t_len: int) -> int:
@@ -487,6 +495,17 @@ class DNATok:
         dnatok_decode(self.h, ids.data_ptr(), out_offsets.data_ptr(), n_rec, out.data_ptr(), int(bytes_capacity), boff.data_ptr(),
                       self._stream(stream))
         return out, boff
+
+    def decode_static(self, ids, out_offsets, out, byte_offsets, stream=None):
+        """decode() into caller-owned buffers with no device allocation anywhere in the call (dnatok_decode_static): out is
+        cuda uint8[bytes_capacity], byte_offsets cuda int64[n_records + 1].  At most DECODE_STATIC_MAX_RECORDS records; calls
+        that overlap on the GPU race on the library's static scratch.  Enqueue only."""
+        t = self._torch
+        assert out.is_cuda and out.dtype == t.uint8 and out.is_contiguous()
+        assert byte_offsets.is_cuda and byte_offsets.dtype == t.int64 and byte_offsets.numel() == out_offsets.numel()
+        dnatok_decode_static(self.h, ids.data_ptr(), out_offsets.data_ptr(), out_offsets.numel() - 1, out.data_ptr(), out.numel(),
+                             byte_offsets.data_ptr(), self._stream(stream))
+        return out, byte_offsets
 
     def embed(self, ids2d, table, b_emb: int = 4096, m_tokens: int = 1 << 20, on_microbatch=None, stream=None):
         """out[r, t, :] = table[ids2d[r, t], :], dnatok_microbatch_rows(b_emb, m_tokens, T) rows per launch.

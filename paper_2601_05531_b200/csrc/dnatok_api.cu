@@ -10,6 +10,7 @@
 #include <cstdint>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <string>
 #include <vector>
 
@@ -23,7 +24,28 @@
 
 using namespace dtk;
 
+// ---- dnatok_decode_static's scratch: decoded bytes per record, DNATOK_DECODE_STATIC_MAX_RECORDS x int32 = 4 MiB, held by
+// every GPU that loads the library until the process exits.  In host code this name is a host-side stand-in, not a device
+// address: the device address of the array on a given GPU comes from cudaGetSymbolAddress with that GPU current
+// (static_scratch_on below), once per device, and is what the kernels are given.
+static __device__ __align__(256) int32_t g_decode_static_rec_len[DNATOK_DECODE_STATIC_MAX_RECORDS];
+
 namespace {
+
+// device address of g_decode_static_rec_len on `device`, which must be the current device; resolved once per device
+int32_t *static_scratch_on(int device) {
+    constexpr int MAX_DEV = 64;
+    static std::mutex mu;
+    static int32_t *addr[MAX_DEV] = {};
+    if (device < 0 || device >= MAX_DEV) return nullptr;
+    std::lock_guard<std::mutex> lock(mu);
+    if (!addr[device]) {
+        void *ptr = nullptr;
+        if (cudaGetSymbolAddress(&ptr, g_decode_static_rec_len) != cudaSuccess || !ptr) { cudaGetLastError(); return nullptr; }
+        addr[device] = static_cast<int32_t *>(ptr);
+    }
+    return addr[device];
+}
 
 // scan scratch of one in-flight encode: tile descriptors, ticket counter, host-mapped status words
 struct EncCtx {
@@ -88,6 +110,7 @@ struct dnatok {
     uint32_t *d_spell_off = nullptr;   // BPE decode: [4 + n_merges + 1] offsets of the token spellings
     uint8_t *d_spell = nullptr;        //             the spellings, back to back (nullptr: too long to keep, decode unavailable)
     int32_t *d_rec_len = nullptr; int64_t rec_len_cap = 0;   // decode: decoded bytes per record
+    int32_t *d_static_rec_len = nullptr;                     // decode_static: device address of g_decode_static_rec_len on h->device
     uint32_t table_mask = 0;
     int32_t bpe_cap = 0;
     EncCtx ctx;
@@ -687,6 +710,8 @@ int dnatok_create(const dnatok_config *cfg_in, int device, dnatok_t **out) {
     cudaDeviceProp prop;
     if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) return bail(DNATOK_ECUDA);
     h->sm_count = prop.multiProcessorCount;
+    h->d_static_rec_len = static_scratch_on(device);          // (the handle's device is current here)
+    if (!h->d_static_rec_len) return bail(DNATOK_ECUDA);
 
     EncParams &p = h->prm;
     p.mode = cfg.mode == DNATOK_KMER ? MODE_KMER : MODE_SINGLE_NT;
@@ -1107,6 +1132,42 @@ int dnatok_decode(dnatok_t *h, const void *d_ids, const int64_t *d_out_offsets, 
     const bool i16 = cfg.id_dtype == DNATOK_I16;
     if (i16) decode_kernel<int16_t, false><<<grid, 256, 0, st>>>(a); else decode_kernel<int32_t, false><<<grid, 256, 0, st>>>(a);
     scan_counts_kernel<<<1, 1024, 0, st>>>(h->d_rec_len, n_records, d_byte_offsets);
+    if (i16) decode_kernel<int16_t, true><<<grid, 256, 0, st>>>(a); else decode_kernel<int32_t, true><<<grid, 256, 0, st>>>(a);
+    CU(cudaGetLastError());
+    h->launches += 3;
+    return DNATOK_OK;
+}
+
+// dnatok_decode without any allocation: the per-record lengths live in the library's static device array.  Nothing in it has
+// to start at zero (the length pass writes every entry the scan reads), so stale contents of an earlier call do no harm; two
+// calls that overlap on the GPU would race on it.
+int dnatok_decode_static(dnatok_t *h, const void *d_ids, const int64_t *d_out_offsets, int64_t n_records, uint8_t *d_bytes_out,
+                         int64_t bytes_capacity, int64_t *d_byte_offsets, void *stream) {
+    if (!h) return DNATOK_EINVAL;
+    if (n_records < 0 || bytes_capacity < 0 || !d_out_offsets || !d_byte_offsets || (bytes_capacity > 0 && !d_bytes_out))
+        return fail(h, DNATOK_EINVAL, "dnatok_decode_static: bad argument");
+    if (n_records > DNATOK_DECODE_STATIC_MAX_RECORDS)
+        return fail(h, DNATOK_ECAPACITY, "dnatok_decode_static: %lld records exceed the static scratch's %d (use dnatok_decode, or split the call)",
+                    (long long)n_records, (int)DNATOK_DECODE_STATIC_MAX_RECORDS);
+    if (h->d_remap4) return fail(h, DNATOK_EINVAL, "dnatok_decode_static: a handle with a k-mer id table has no inverse table");
+    if (h->cfg.mode == DNATOK_BPE && !h->d_spell)
+        return fail(h, DNATOK_EINVAL, "dnatok_decode_static: the merge table's token spellings exceed 64 MiB");
+    USE_DEVICE(h);
+    cudaStream_t st = (cudaStream_t)stream;
+    const dnatok_config &cfg = h->cfg;
+    DecodeArgs a;
+    a.ids = d_ids; a.out_off = d_out_offsets; a.n_rec = n_records;
+    a.mode = cfg.mode; a.k = cfg.mode == DNATOK_KMER ? cfg.k : 1; a.base_id = cfg.base_id; a.n_id = cfg.n_id; a.pad_id = cfg.pad_id;
+    for (int i = 0; i < 5; ++i) a.nt_ids[i] = cfg.nt_ids[i];
+    a.four_k = 1ll << (2 * a.k);
+    a.n_tokens_bpe = 4 + cfg.n_merges; a.spell_off = h->d_spell_off; a.spell = h->d_spell;
+    a.rec_len = h->d_static_rec_len; a.byte_off = d_byte_offsets; a.out = d_bytes_out; a.out_cap = bytes_capacity;
+    a.status = h->ctx.d_status;
+    int grid = (int)std::min<int64_t>((n_records + 7) / 8 + 1, (int64_t)h->sm_count * 8);
+    if (h->grid_cap > 0) grid = std::min(grid, h->grid_cap);
+    const bool i16 = cfg.id_dtype == DNATOK_I16;
+    if (i16) decode_kernel<int16_t, false><<<grid, 256, 0, st>>>(a); else decode_kernel<int32_t, false><<<grid, 256, 0, st>>>(a);
+    scan_counts_kernel<<<1, 1024, 0, st>>>(h->d_static_rec_len, n_records, d_byte_offsets);
     if (i16) decode_kernel<int16_t, true><<<grid, 256, 0, st>>>(a); else decode_kernel<int32_t, true><<<grid, 256, 0, st>>>(a);
     CU(cudaGetLastError());
     h->launches += 3;
