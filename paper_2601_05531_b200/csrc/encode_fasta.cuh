@@ -28,14 +28,25 @@ namespace fa {
 
 using namespace dtk::v5;
 
-constexpr int FW_CHUNKS = 8;                        // 2 KiB chunks per warp tile
+// (compile-time knobs for tuning sweeps -- DTK_NVCC_FLAGS="-DFW_WARPS_N=4 -DFW_CHUNKS_N=6 -DFW_MINB=7" -- the defaults are the
+// measured optimum)
+#ifndef FW_CHUNKS_N
+#define FW_CHUNKS_N 8
+#endif
+#ifndef FW_WARPS_N
+#define FW_WARPS_N 8
+#endif
+#ifndef FW_MINB
+#define FW_MINB 3
+#endif
+constexpr int FW_CHUNKS = FW_CHUNKS_N;               // 2 KiB chunks per warp tile
 constexpr int FW_TILE = FW_CHUNKS * WB;             // bytes per warp tile (16 KiB)
 constexpr int FW_HALO = 64;                         // bytes read past a piece that ends at the tile's end
 constexpr int FW_BASES = FW_TILE + FW_HALO;
 constexpr int FW_CW = FW_BASES / 16 + 8;            // code words of a warp's stream (+ over-read slack)
 constexpr int FW_FW = FW_BASES / 32 + 10;
 constexpr int FW_WORDS = FW_CW + FW_FW;
-constexpr int FW_WARPS = 8;                         // warps per CTA
+constexpr int FW_WARPS = FW_WARPS_N;                 // warps per CTA
 constexpr int FW_MAXSEG = 2 * FW_CHUNKS;            // records per warp tile the fast path accepts
 constexpr int FW_HDR_BOUND = 4096;                  // bytes the parse reads looking for the end of a header line
 constexpr int FW_LINE_BOUND = 512;                  //   ... and for the end of the first sequence line
@@ -390,7 +401,7 @@ __device__ __forceinline__ int clamp64(int64_t v) { return v < 0 ? 0 : (v > 64 ?
 // KK: the emission variant compiled in -- 0 single-nt, 1..6 / 8 that k, -1 every variant behind a run-time switch
 // FUSED: the tokens go into the padded batch (FastaArgs::seq_len > 0; IdT = int32_t)
 template <typename IdT, int KK, bool FUSED = false>
-__global__ void __launch_bounds__(FW_WARPS * 32, 3) encode_fasta_kernel(const __grid_constant__ FastaArgs F) {
+__global__ void __launch_bounds__(FW_WARPS * 32, FW_MINB) encode_fasta_kernel(const __grid_constant__ FastaArgs F) {
     extern __shared__ __align__(16) uint8_t smem_raw[];
     SmemFa &sm = *reinterpret_cast<SmemFa *>(smem_raw);
     constexpr uint32_t FULL = 0xffffffffu;
@@ -403,7 +414,7 @@ __global__ void __launch_bounds__(FW_WARPS * 32, 3) encode_fasta_kernel(const __
     const bool affine = P.nt_ids[1] == P.nt_ids[0] + 1 && P.nt_ids[2] == P.nt_ids[0] + 2 && P.nt_ids[3] == P.nt_ids[0] + 3;
     const bool vec_ok = (reinterpret_cast<uintptr_t>(A.ids) & 15) == 0 &&
                         (P.mode != MODE_KMER || (k >= 1 && k <= 6) || k == 8);
-    sm.lut[tid] = A.lut[tid];
+    for (int i = tid; i < 256; i += FW_WARPS * 32) sm.lut[i] = A.lut[i];
     __syncthreads();
     asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
     asm volatile("griddepcontrol.wait;" ::: "memory");           // par, wt_first, out_offsets come from the kernels in front
