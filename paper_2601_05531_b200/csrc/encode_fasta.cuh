@@ -417,6 +417,11 @@ __global__ void __launch_bounds__(FW_WARPS * 32, FW_MINB) encode_fasta_kernel(co
     for (int i = tid; i < 256; i += FW_WARPS * 32) sm.lut[i] = A.lut[i];
     __syncthreads();
     asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+    {   // the warp's first tile on its way to L2 while the parse and scan kernels in front still run (HBM idles meanwhile)
+        const int64_t p0 = ((int64_t)blockIdx.x * FW_WARPS + warp) * FW_TILE;
+        int64_t sz = A.p_end - p0; if (sz > FW_TILE) sz = FW_TILE; sz &= ~(int64_t)15;
+        if (lane == 0 && sz > 0) asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(A.bytes_al + p0), "r"((uint32_t)sz) : "memory");
+    }
     asm volatile("griddepcontrol.wait;" ::: "memory");           // par, wt_first, out_offsets come from the kernels in front
     uint32_t *const cw = sm.strm[warp], *const fw = cw + FW_CW;
     IdT *const ids = reinterpret_cast<IdT *>(A.ids);

@@ -29,6 +29,13 @@ __global__ void __launch_bounds__(NT7, 3) encode_tiles_v7(const __grid_constant_
     if (tid < 256) sm.lut[tid] = A.lut[tid];
     // launched with programmatic stream serialisation: everything above overlaps the tail of the pre-pass kernel, whose
     // outputs (first_rec, out_offsets) are read only behind this point (a no-op in an ordinary launch)
+    // ... and so does the fetch of the tile this CTA will most likely draw first (tickets go out in launch order), as a hint
+    // to L2: the input bytes are nobody's output, and HBM idles while the pre-pass runs
+    if (tid < A.S) {
+        const int64_t p0 = ((int64_t)blockIdx.x * A.S + tid) * TB;
+        int64_t sz = A.p_end - p0; if (sz > TB) sz = TB; sz &= ~(int64_t)15;
+        if (sz > 0) asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(A.bytes_al + p0), "r"((uint32_t)sz) : "memory");
+    }
     asm volatile("griddepcontrol.wait;" ::: "memory");
     if (tid == 0) sm.done_cnt = 0;
     __syncthreads();
