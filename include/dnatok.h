@@ -279,6 +279,10 @@ int dnatok_set_super_tile(dnatok_t *h, int32_t sub_tiles);
  * encoder first, which assumes records laid out as an optional '>' header line followed by lines of one fixed width and
  * checks that layout on every byte; the chained-scan encoder runs behind it only if the check failed somewhere.  2 = the
  * same for inputs of any size (tests), 0 = the chained-scan encoder only.  Results never depend on it.  EINVAL outside 0..2.
+ * With 1, two host-side rules keep hopeless attempts away: an input that averages more than 8 records per 16 KiB goes to the
+ * chained-scan encoder directly, and after a call whose check failed (it then cost both encoders' time) the next 8 eligible
+ * calls on the handle do too; the failure is read from a host-mapped word without synchronising, so it may take effect a
+ * call or two late.
  */
 int dnatok_set_fast_path(dnatok_t *h, int32_t enable);
 

@@ -58,7 +58,8 @@ struct EncCtx {
     int64_t reck_cap = 0;
     unsigned long long *ticket = nullptr;
     unsigned long long ticket_base = 0;
-    uint32_t *h_status = nullptr;      // pinned + mapped: [0] capacity overflow, [1] scan protocol failure
+    uint32_t *h_status = nullptr;      // pinned + mapped: [0] capacity overflow, [1] scan protocol failure, [2] a layout check failed
+    int fa_skip = 0;                   // calls left that go to the chained-scan encoder directly after a failed layout check
     uint32_t *d_status = nullptr;      // device alias of h_status
     uint32_t gen = 0;
     unsigned long long *prof = nullptr;   // phase timers of debug builds (-DDTK_PROF)
@@ -171,8 +172,8 @@ uint32_t host_hash(uint32_t key) {   // must match bpe_hash()
 int ctx_init(dnatok_t *h, EncCtx &c) {
     CU(cudaMalloc(&c.ticket, sizeof(unsigned long long)));
     CU(cudaMemset(c.ticket, 0, sizeof(unsigned long long)));
-    CU(cudaHostAlloc(&c.h_status, 2 * sizeof(uint32_t), cudaHostAllocMapped));
-    c.h_status[0] = c.h_status[1] = 0;
+    CU(cudaHostAlloc(&c.h_status, 4 * sizeof(uint32_t), cudaHostAllocMapped));
+    c.h_status[0] = c.h_status[1] = c.h_status[2] = c.h_status[3] = 0;
     CU(cudaHostGetDevicePointer((void **)&c.d_status, c.h_status, 0));
     CU(cudaMalloc(&c.prof, 64 * sizeof(unsigned long long)));
     CU(cudaMemset(c.prof, 0, 64 * sizeof(unsigned long long)));
@@ -287,6 +288,7 @@ void launch_pdl1(K kernel, int grid, int block, size_t smem, cudaStream_t st, bo
 // The regular-layout path costs three launches and a latency-bound parse before its encoder starts; measured against the
 // chained-scan encoder on L2-flushed inputs of both FASTA shapes it wins from 32-64 MiB on.
 constexpr int64_t FAST_PATH_MIN_BYTES = 48ll << 20;
+constexpr int FAST_PATH_SKIP_CALLS = 8;
 
 template <typename IdT, bool FUSED = false>
 void launch_fasta(const fa::FastaArgs &f, int kk, int grid, cudaStream_t st) {
@@ -373,7 +375,16 @@ int launch_tiles(dnatok_t *h, EncCtx &c, const EncParams &prm, const uint8_t *d_
         bool chained = false;                                 // the kernels below follow kernels of this call
         bool f_fused = false;
         c.fa_tried = false;
-        if ((h->fast_path == 2 || (h->fast_path == 1 && n_bytes >= FAST_PATH_MIN_BYTES)) && n_rec < (1ll << 31)) {
+        // (many short records: more than FW_MAXSEG of them would meet in some 16 KiB tile and fail the layout check anyway,
+        // so an input that averages over half of that goes to the chained-scan encoder directly)
+        const bool short_recs = h->fast_path != 2 && n_rec > (n_bytes / fa::FW_TILE + 1) * (fa::FW_MAXSEG / 2);
+        // A failed layout check costs the regular-layout encoder's time on top of the chained scan's.  Inputs of one source tend
+        // to be alike, so after a failure (reported by the fall-back launch through a host-mapped word; read here without any
+        // synchronisation, so it may be seen a call or two late) the next FAST_PATH_SKIP_CALLS calls on this context skip the attempt.
+        if (((volatile uint32_t *)c.h_status)[2]) { c.h_status[2] = 0; c.fa_skip = FAST_PATH_SKIP_CALLS; }
+        bool try_fast = (h->fast_path == 2 || (h->fast_path == 1 && n_bytes >= FAST_PATH_MIN_BYTES)) && n_rec < (1ll << 31) && !short_recs;
+        if (try_fast && h->fast_path == 1 && c.fa_skip > 0) { --c.fa_skip; try_fast = false; }
+        if (try_fast) {
             // regular-layout fast path first (encode_fasta.cuh); the chained-scan encoder behind it runs only if the layout
             // check failed somewhere
             const int64_t n_wtiles = (a.p_end + fa::FW_TILE - 1) / fa::FW_TILE;

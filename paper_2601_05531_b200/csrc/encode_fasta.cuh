@@ -441,6 +441,8 @@ __global__ void __launch_bounds__(FW_WARPS * 32, FW_MINB) encode_fasta_kernel(co
     int64_t tile = (int64_t)blockIdx.x * FW_WARPS + warp;
 #pragma unroll 1
     while (tile < F.n_wtiles) {
+        // somebody has found the layout irregular: the chained-scan encoder will redo everything, so stop here
+        if (__ldcg(F.irregular) != 0u) break;
         int64_t next_tile = 0;
         if (lane == 0) next_tile = n_warps + (int64_t)atomicAdd(tile_ctr, 1ull);
         next_tile = __shfl_sync(FULL, next_tile, 0);
@@ -851,6 +853,7 @@ __global__ void __launch_bounds__(FW_WARPS * 32, FW_MINB) encode_fasta_kernel(co
             }
             __syncwarp();
         }
+        if (__any_sync(FULL, irregular)) break;                     // published below; the other warps stop at their next tile
         tile = next_tile;
     }
     if (__any_sync(FULL, irregular) && lane == 0) *F.irregular = 1u;

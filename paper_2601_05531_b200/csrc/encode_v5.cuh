@@ -689,6 +689,9 @@ __global__ void __launch_bounds__(NT, 1024 / NT) encode_tiles_v5(const __grid_co
         if (blockIdx.x == 0 && tid == 0) atomicAdd(A.ticket, (unsigned long long)A.n_tiles + gridDim.x);
         return;
     }
+    // this launch redoes an input whose layout check failed: tell the host (status word 2, read without synchronising at its
+    // next call), which then leaves the regular-layout encoder out for a while
+    if (A.run_if && blockIdx.x == 0 && tid == 0) A.status[2] = 1u;
     __syncthreads();
     unsigned long long next_ticket = 0;
     if (warp == NW - 1) {

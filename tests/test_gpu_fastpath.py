@@ -391,3 +391,40 @@ def test_fused_entry_point_serves_bpe_and_dense_specs_through_the_pad_kernel():
     lut = oracle.default_lut().copy()
     lut[lut == oracle.CLS_SKIP] = oracle.CLS_UNK                               # no SKIP class + no header strip: the dense encoder
     run_padded(b"".join(recs), offs, False, 64, 1, mode="kmer", k=3, class_lut=lut, strip_headers=False)
+
+
+def test_after_a_failed_layout_check_the_next_calls_skip_the_attempt():
+    """dnatok_set_fast_path(1), the default: a fall-back is reported to the host, which then sends the next 8 eligible calls on the
+    handle to the chained-scan encoder directly (results are the oracle's either way)"""
+    import dnagen
+    dn.FAST_PATH = 1
+    w = dnagen.config3(total_bases=50 << 20, lo=1000, hi=131072, seed=31)       # over the 48 MiB threshold
+    bad = w.data.copy()
+    p = bad.size // 3
+    p += int(bad[p] == 10)
+    bad[p] = 13                                                                # one '\r' inside a line
+    cfg = oracle.Config(mode=oracle.KMER, k=6)
+    want_ok, want_off_ok = oracle.encode(w.data, w.offsets, cfg)
+    want_bad, want_off_bad = oracle.encode(bad, w.offsets, cfg)
+    tok = dn.DNATok(mode="kmer", k=6)
+    d_ok, d_bad = torch.from_numpy(w.data).cuda(), torch.from_numpy(bad).cuda()
+    o = torch.from_numpy(w.offsets).cuda()
+
+    def call(d, want, want_off):
+        ids, out = tok.encode(d, o)
+        tok.check()
+        taken = tok.fast_path_taken()
+        out = out.cpu().numpy()
+        assert np.array_equal(out, want_off) and np.array_equal(ids[: out[-1]].cpu().numpy(), want)
+        return taken
+
+    assert call(d_ok, want_ok, want_off_ok) is True
+    assert call(d_bad, want_bad, want_off_bad) is False                        # tried, failed, redone by the chained scan
+    skipped = [call(d_ok, want_ok, want_off_ok) for _ in range(8)]
+    assert skipped == [False] * 8                                              # not even tried
+    assert call(d_ok, want_ok, want_off_ok) is True                            # ... and tried again afterwards
+    small = w.data[: int(w.offsets[5])]
+    tok2 = dn.DNATok(mode="kmer", k=6)
+    ids, out = tok2.encode(torch.from_numpy(small.copy()).cuda(), torch.from_numpy(w.offsets[:6].copy()).cuda())
+    tok2.check()
+    assert tok2.fast_path_taken() is False                                     # under the threshold: never tried
