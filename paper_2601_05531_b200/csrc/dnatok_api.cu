@@ -402,7 +402,7 @@ int launch_tiles(dnatok_t *h, EncCtx &c, const EncParams &prm, const uint8_t *d_
                 f.seq_len = h->cfg.seq_len; f.pad_side = h->cfg.pad_side;
                 f.e.ids = d_batch; f.e.ids_cap = n_rec * (int64_t)h->cfg.seq_len;
             }
-            const int64_t nthr = std::max<int64_t>(n_rec, n_wtiles);
+            const int64_t nthr = n_rec + n_wtiles;                       // one thread per tile, then one per record
             fa::fasta_parse_kernel<<<(unsigned)std::max<int64_t>(1, (nthr + 255) / 256), 256, 0, st>>>(f);
             launch_pdl1(fa::offsets_scan_kernel, (int)nb_scan, fa::OS_NT, 0, st, true, (const int32_t *)c.fa_tok, n_rec, out_off, (int64_t)0, c.descs, a.gen, c.d_status);
             int fgrid = (int)std::min<int64_t>((n_wtiles + fa::FW_WARPS - 1) / fa::FW_WARPS, (int64_t)h->sm_count * h->fasta_ctas_per_sm);

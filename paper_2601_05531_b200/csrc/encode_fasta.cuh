@@ -125,9 +125,12 @@ __device__ __forceinline__ int64_t find_nl(const uint8_t *al, int64_t from, int6
 __global__ void __launch_bounds__(256) fasta_parse_kernel(const __grid_constant__ FastaArgs F) {
     const EncArgs &A = F.e;
     const EncParams &P = A.prm;
-    const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    // threads [0, n_wtiles) search for the first record of a tile, threads [n_wtiles, n_wtiles + n_rec) parse a record each: two
+    // short chains of dependent loads side by side instead of one long one per thread
+    const int64_t t0 = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
-    if (t < F.n_wtiles) {
+    if (t0 < F.n_wtiles) {
+        const int64_t t = t0;
         // last record whose start is at or before the tile's first byte (0 if the tile starts in front of every record)
         const int64_t pos = t * FW_TILE;
         // number of offsets <= pos, by a 16-way search: the 16 probes of a step are independent loads, so the chain of
@@ -147,7 +150,9 @@ __global__ void __launch_bounds__(256) fasta_parse_kernel(const __grid_constant_
             if (c < 16 && nhi < hi) hi = nhi;
         }
         F.wt_first[t] = (int32_t)(lo > 0 ? lo - 1 : 0);
+        return;
     }
+    const int64_t t = t0 - F.n_wtiles;
     if (t >= A.n_rec) return;
     const int64_t a = rec_pos(A, t), e = rec_pos(A, t + 1), L = e - a;
     const uint8_t *b = A.bytes_al + a;
