@@ -469,8 +469,15 @@ def bench_config(dn, torch, D: Dist, local: int, config: int, k: int, args, *, e
         kname = "encode_fasta_kernel"                            # the regular-layout encoder served the call (dnatok.h)
     roof = {"bound": "hbm", "kernel": kname, "achieved": alg_bytes / (kern_ms * 1e-3) / 1e9, "peak": peak, "unit": "GB/s",
             "peak_source": peak_src, "algorithmic_bytes_per_launch": alg_bytes,
-            "bytes_per_base": alg_bytes / max(1, bases), "kernel_ms": kern_ms,
-            "traffic": args.traffic if args.traffic is not None else committed_profile(f"config{config}")}
+            "bytes_per_base": alg_bytes / max(1, bases), "kernel_ms": kern_ms, "traffic": args.traffic}
+    if args.traffic is None:
+        # a committed ncu capture counts as this launch's DRAM traffic only if it is OF this launch: full size, and for config 3
+        # the k = 6 kernel; config 5 was captured at an eighth of its size (profiles/r2_pad.md) and is reported as such
+        if args.scale == 1.0 and config != 5 and (config != 3 or k == 6):
+            roof["traffic"] = committed_profile(f"config{config}")
+        elif config == 5:
+            roof["traffic_at_scale"] = {"scale": 0.125, "dram_bytes": committed_profile("config5"), "method_bytes": 2416e6,
+                                        "source": "profiles/r2_pad.md"}
     roof["frac"] = roof["achieved"] / peak
     if L:
         if kname == "encode_fasta_kernel":
