@@ -432,10 +432,6 @@ __global__ void __launch_bounds__(FW_WARPS * 32, FW_MINB) encode_fasta_kernel(co
     IdT *const ids = reinterpret_cast<IdT *>(A.ids);
     bool irregular = false;
     const bool nl_skips = sm.lut[(uint8_t)'\n'] == CLS_SKIP;
-    // x >> 1 and x >> 2 as multiply-high by 2^31 and 2^30: the shifts of the classification leave the ALU pipe, which bounds
-    // this kernel, for the FMA pipe, which idles (IMAD.HI issues at half rate, measured, and overlaps LOP3 fully).  The factors
-    // are kept opaque so that the compiler does not turn the multiplies back into shifts.
-    const uint32_t mh31 = 0x80000000u | (uint32_t)(F.n_wtiles < 0), mh30 = mh31 >> 1;
 
     // Tiles are handed out through a counter (F.irregular + 2, zeroed with the flag): the first one of a warp is its own index,
     // every later one is taken when the warp starts the tile before it, so that no SM is left idle while others still have
@@ -600,7 +596,7 @@ __global__ void __launch_bounds__(FW_WARPS * 32, FW_MINB) encode_fasta_kernel(co
                         for (int j = 0; j < 16; ++j) {
                             const uint32_t x = xw[j];
                             cb[j] = (x & 0x06060606u) * 0x00820820u;
-                            const uint32_t m = __umulhi(x, mh30) & ~__umulhi(x, mh31) & 0x01010101u;
+                            const uint32_t m = (x >> 2) & ~(x >> 1) & 0x01010101u;       // (as IMAD.HI on the FMA pipe: 1 % slower)
                             dd[j] = (x & 0xD9D9D9D9u) ^ (m * 0x0fu + 0x41414141u);
                         }
 #pragma unroll
